@@ -1,0 +1,150 @@
+/*
+ * bb.h -- C ABI of libbiobeam_b200.so: the split-step beam-propagation (BPM) hot path of
+ * biobeam (arxiv 1706.02261), hand-written for NVIDIA B200 (sm_100a).
+ *
+ * What the library computes.  The paper's main text names the method (PAPER.md line 21:
+ * "beam-propagation model (BPM) ... we use the exact propagator together with a locally
+ * adapted expansion of refractive indices", and the "novel multiplexing scheme" that
+ * propagates 100s-1000s of point sources in one field); its formulas are in supplementary
+ * notes that are not available, so the per-slice operations are the ones
+ * BASELINE.json:north_star states, with the readings listed in DESIGN.md ("Readings"):
+ *
+ *   for j = 0 .. Nz-1:                                    (reading A5, A6)
+ *       U  = FFT2(u)                                      unnormalised, kernel exp(-i k.r)
+ *       U *= (s > 0) ? exp(+i dz sqrt(s)) : 0             s = k^2 - kx^2 - ky^2,  k = k0 n_ref[j]
+ *       u  = IFFT2(U)                                     with 1/(Nx Ny)
+ *       u *= exp(+i k0 dz (n0 + dn[j] - n_ref[j]))        k0 = 2 pi / lambda
+ *       I[j] = sum over batch |u|^2                       (or per field / accumulated)
+ *
+ *   kx[p] = 2 pi (p < Nx/2 ? p : p - Nx) / (Nx dx), likewise ky with Ny and dy = dx.
+ *
+ * Conventions.  All lengths in micrometres; lambda is the vacuum wavelength.  Arrays are
+ * row-major with x fastest: field [B][Ny][Nx] of float pairs (re, im) = complex64,
+ * volumes [Nz][Ny][Nx] float32.  Scalars are float32; every table is built in double from
+ * the float32 values promoted to double.  Nx and Ny must be powers of two in [32, 1024]
+ * (Nx != Ny allowed).  Periodic lateral boundaries (plain FFT).
+ *
+ * Pointers.  Unless a parameter says HOST, pointers are DEVICE pointers on the current CUDA
+ * device (e.g. torch tensor data_ptr()).  The caller owns every buffer in a signature; the
+ * library owns only its plan cache (twiddle tables, propagator tables, a few KB of
+ * workspace), created lazily and released by bb_shutdown().  The library never copies user
+ * data between host and device except in bb_propagate_host() and for the small HOST arrays.
+ *
+ * Execution.  Device-pointer calls enqueue work on the given stream and return without
+ * waiting for it (they may synchronise the first time a shape or reference index is seen,
+ * while tables are built).  Calls on one device must not overlap on different streams.
+ * There is no CPU fallback and no other backend: on a device that is not sm_100 every
+ * compute call returns BB_ERR_ARCH.
+ *
+ * Errors.  Every call returns a bb_status; nothing throws or aborts.  Arguments are
+ * checked before any launch.  bb_last_error() returns a thread-local message for the last
+ * non-OK status.
+ */
+#ifndef BIOBEAM_B200_BB_H
+#define BIOBEAM_B200_BB_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    BB_OK = 0,
+    BB_ERR_INVALID_ARG = 1,        /* NULL pointer, non-positive scalar, bad count, bad flags */
+    BB_ERR_UNSUPPORTED_SHAPE = 2,  /* Nx or Ny not a power of two in [32, 1024] */
+    BB_ERR_CUDA = 3,               /* a CUDA call failed (message in bb_last_error) */
+    BB_ERR_OOM = 4,                /* device or host allocation failed */
+    BB_ERR_ARCH = 5,               /* current device is not compute capability 10.x */
+    BB_ERR_INTERNAL = 6            /* device-side watchdog tripped (grid barrier timeout) */
+} bb_status;
+
+/* bb_opts.flags */
+#define BB_ACCUMULATE          1u  /* intensity_out += |u|^2 instead of = (reading A11) */
+#define BB_INTENSITY_PER_FIELD 2u  /* intensity_out is [B][Nz][Ny][Nx], not summed over the batch */
+#define BB_LAUNCH_PER_PHASE    4u  /* diagnostic: one kernel launch per half-step instead of one
+                                      persistent cooperative kernel (same arithmetic, same results) */
+
+typedef struct {
+    int struct_size;     /* sizeof(bb_opts); lets the struct grow compatibly */
+    int batch;           /* B >= 1 independent fields, contiguous [B][Ny][Nx], one shared dn volume
+                            (north_star item 4, BASELINE.json configs[4]) */
+    const float *nref;   /* HOST float[Nz]: reference index n_ref[j] of step j (reading A3),
+                            or NULL = n0 for every step */
+    unsigned flags;      /* BB_ACCUMULATE | BB_INTENSITY_PER_FIELD | BB_LAUNCH_PER_PHASE */
+    void *stream;        /* cudaStream_t; NULL = the legacy default stream */
+} bb_opts;
+
+/*
+ * bb_propagate -- north_star: "bb_propagate(field, dn_volume, Nx, Ny, Nz, dx, dz, lambda, n0,
+ * intensity_out)".  Algorithm above with B = 1, n_ref = n0, flags = 0, default stream.
+ *   field          in: u at the input plane z = 0; out: u after Nz steps (in place)
+ *   dn_volume      float[Nz][Ny][Nx] = n - n0; step j uses slice j
+ *   intensity_out  float[Nz][Ny][Nx], slice j = |u|^2 after step j (z = (j+1) dz); may be NULL
+ */
+int bb_propagate(void *field, const float *dn_volume, int Nx, int Ny, int Nz,
+                 float dx, float dz, float lambda, float n0, float *intensity_out);
+
+/* Same with options (batch, adapted n_ref, accumulate / per-field intensity, stream). opts may be NULL. */
+int bb_propagate_ex(void *field, const float *dn_volume, int Nx, int Ny, int Nz,
+                    float dx, float dz, float lambda, float n0, float *intensity_out,
+                    const bb_opts *opts);
+
+/*
+ * bb_propagate_host -- the same computation for HOST buffers: field, dn_volume and
+ * intensity_out are HOST pointers (pinned memory gives overlap of the copies with the
+ * kernels; pageable memory works but serialises).  The dn volume is streamed to the device
+ * in z-chunks while earlier chunks are computed and their intensity slices are streamed back;
+ * every step still runs in the CUDA kernels.  Synchronous: returns when the results are in
+ * host memory.  opts->stream is ignored (the call owns its streams).
+ */
+int bb_propagate_host(void *field_host, const float *dn_volume_host, int Nx, int Ny, int Nz,
+                      float dx, float dz, float lambda, float n0, float *intensity_out_host,
+                      const bb_opts *opts);
+
+/*
+ * bb_nref_from_dn -- locally adapted reference index ("locally adapted
+ * expansion of refractive indices"; reading A3): n_ref[j] = n0 + mean of dn over the slab of
+ * `slab` consecutive slices that contains j (the last slab may be short), means in double,
+ * result rounded to float32.  dn is a DEVICE pointer, nref_out a HOST float[Nz].
+ * Synchronises the stream.
+ */
+int bb_nref_from_dn(const float *dn_volume, int Nx, int Ny, int Nz, float n0, int slab,
+                    float *nref_out_host, void *stream);
+
+/*
+ * bb_multiplex_psf -- north_star: "bb_multiplex_psf(emitter_positions, NA, ...)"; PAPER.md
+ * line 21 ("sets of 100s to 1000s of mutually independent ... PSFs ... within single, highly
+ * multiplexed simulations") and line 29 ("multiplexed diffraction-limited point-sources").
+ * Readings A12-A14:
+ *   P[q][p]  = 1 if kx^2 + ky^2 <= (k0 NA)^2 else 0
+ *   U0[q][p] = P * sum_e a_e exp(i (phi_e - kx X_e - ky Y_e)),  X_e = x_e + (Nx/2) dx, Y_e likewise
+ *   field    = IFFT2(U0) * (Nx Ny / sum P)          (an on-grid unit emitter has field 1 at its pixel)
+ *   emitter_positions  float[M][2] (x, y) in um, origin at pixel (Nx/2, Ny/2)
+ *   emitter_phase      float[M] rad, or NULL = 0;   emitter_amp  float[M], or NULL = 1
+ *   field_out          float pairs [Ny][Nx]
+ */
+int bb_multiplex_psf(const float *emitter_positions, const float *emitter_phase,
+                     const float *emitter_amp, int M, float NA,
+                     int Nx, int Ny, float dx, float lambda, void *field_out, void *stream);
+
+/*
+ * Building blocks, exported so that each can be checked against the oracle on its own.
+ * bb_fft2: in-place 2-D DFT of `batch` fields; sign = -1 forward (unnormalised), +1 inverse
+ * (divides by Nx Ny).  bb_propagator_table: the table the propagator multiply uses,
+ * H[q][p] = (s > 0 ? exp(i dz sqrt(s)) : 0) / (Nx Ny) as float pairs [Ny][Nx] (the 1/(Nx Ny) of
+ * the inverse transform is folded in; a power of two, so exact).
+ */
+int bb_fft2(void *field, int Nx, int Ny, int batch, int sign, void *stream);
+int bb_propagator_table(int Nx, int Ny, float dx, float dz, float lambda, float nref,
+                        void *table_out, void *stream);
+
+const char *bb_last_error(void);        /* thread-local; "" if none */
+int bb_version(void);                   /* 100 * major + minor */
+void bb_shutdown(void);                 /* frees cached plans, tables and workspace (synchronises) */
+unsigned long long bb_launch_count(void); /* kernels launched by this library since load */
+int bb_device_status(void);             /* synchronises the device; BB_ERR_INTERNAL if a device-side
+                                           watchdog tripped since the last call, else BB_OK */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BIOBEAM_B200_BB_H */

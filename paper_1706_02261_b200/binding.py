@@ -1,0 +1,209 @@
+"""ctypes binding of ``libbiobeam_b200.so`` (``include/bb.h``): argument marshalling only.
+
+Every function takes torch tensors (device memory and streams are torch's; all arithmetic
+runs in the library's CUDA kernels) and has the name of the C entry point without ``bb_``.
+There is no fallback: if the shared library is missing or a call fails, an exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libbiobeam_b200.so")
+
+ACCUMULATE = 1
+INTENSITY_PER_FIELD = 2
+LAUNCH_PER_PHASE = 4
+
+EXPORTS = ("bb_propagate", "bb_propagate_ex", "bb_propagate_host", "bb_nref_from_dn",
+           "bb_multiplex_psf", "bb_fft2", "bb_propagator_table", "bb_last_error", "bb_version",
+           "bb_shutdown", "bb_launch_count", "bb_device_status")
+
+STATUS_NAMES = {0: "BB_OK", 1: "BB_ERR_INVALID_ARG", 2: "BB_ERR_UNSUPPORTED_SHAPE", 3: "BB_ERR_CUDA",
+                4: "BB_ERR_OOM", 5: "BB_ERR_ARCH", 6: "BB_ERR_INTERNAL"}
+
+
+class BBError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__("%s: %s" % (STATUS_NAMES.get(status, str(status)), message))
+        self.status = status
+
+
+class _Opts(ctypes.Structure):
+    _fields_ = [("struct_size", ctypes.c_int), ("batch", ctypes.c_int),
+                ("nref", ctypes.POINTER(ctypes.c_float)), ("flags", ctypes.c_uint),
+                ("stream", ctypes.c_void_p)]
+
+
+_lib = None
+
+
+def load() -> ctypes.CDLL:
+    """Loads the shared library (built by ``paper_1706_02261_b200.build``); raises if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise FileNotFoundError(
+            "%s not found: build it with `python -m paper_1706_02261_b200.build` "
+            "(there is no fallback implementation)" % LIB_PATH)
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, fp, i, f = ctypes.c_void_p, ctypes.POINTER(ctypes.c_float), ctypes.c_int, ctypes.c_float
+    lib.bb_propagate.argtypes = [vp, vp, i, i, i, f, f, f, f, vp]
+    lib.bb_propagate_ex.argtypes = [vp, vp, i, i, i, f, f, f, f, vp, ctypes.POINTER(_Opts)]
+    lib.bb_propagate_host.argtypes = [vp, vp, i, i, i, f, f, f, f, vp, ctypes.POINTER(_Opts)]
+    lib.bb_nref_from_dn.argtypes = [vp, i, i, i, f, i, fp, vp]
+    lib.bb_multiplex_psf.argtypes = [vp, vp, vp, i, f, i, i, f, f, vp, vp]
+    lib.bb_fft2.argtypes = [vp, i, i, i, i, vp]
+    lib.bb_propagator_table.argtypes = [i, i, f, f, f, f, vp, vp]
+    lib.bb_last_error.restype = ctypes.c_char_p
+    lib.bb_launch_count.restype = ctypes.c_ulonglong
+    lib.bb_shutdown.restype = None
+    _lib = lib
+    return lib
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise BBError(rc, load().bb_last_error().decode("utf-8", "replace"))
+
+
+def _stream_ptr(stream) -> Optional[int]:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+def _field_shape(field: torch.Tensor):
+    if field.dtype != torch.complex64 or not field.is_contiguous():
+        raise TypeError("field must be a contiguous complex64 tensor [B][Ny][Nx] or [Ny][Nx]")
+    if field.dim() == 2:
+        return 1, field.shape[0], field.shape[1]
+    if field.dim() == 3:
+        return field.shape[0], field.shape[1], field.shape[2]
+    raise TypeError("field must be [B][Ny][Nx] or [Ny][Nx]")
+
+
+def _f32(t: torch.Tensor, name: str):
+    if t.dtype != torch.float32 or not t.is_contiguous():
+        raise TypeError("%s must be a contiguous float32 tensor" % name)
+    return t
+
+
+def propagate(field: torch.Tensor, dn: torch.Tensor, dx: float, dz: float, lam: float, n0: float,
+              intensity: Optional[torch.Tensor] = None, nref=None, flags: int = 0, stream=None):
+    """``bb_propagate_ex`` (CUDA tensors; asynchronous on ``stream``) or ``bb_propagate_host``
+    (CPU tensors, pinned for overlap; synchronous).  ``field`` is updated in place.
+    ``nref``: None or a sequence / CPU tensor of Nz floats."""
+    lib = load()
+    B, Ny, Nx = _field_shape(field)
+    _f32(dn, "dn")
+    if dn.dim() != 3 or dn.shape[1] != Ny or dn.shape[2] != Nx:
+        raise TypeError("dn must be [Nz][%d][%d]" % (Ny, Nx))
+    Nz = dn.shape[0]
+    on_gpu = field.is_cuda
+    if dn.is_cuda != on_gpu or (intensity is not None and intensity.is_cuda != on_gpu):
+        raise TypeError("field, dn and intensity must all be CUDA tensors or all CPU tensors")
+    if intensity is not None:
+        _f32(intensity, "intensity")
+        want = (B * Nz if flags & INTENSITY_PER_FIELD else Nz) * Ny * Nx
+        if intensity.numel() != want:
+            raise TypeError("intensity has %d elements, expected %d" % (intensity.numel(), want))
+    opts = _Opts()
+    opts.struct_size = ctypes.sizeof(_Opts)
+    opts.batch = B
+    opts.flags = flags
+    nref_buf = None
+    if nref is not None:
+        nref_buf = (ctypes.c_float * Nz)(*[float(x) for x in nref])
+        opts.nref = ctypes.cast(nref_buf, ctypes.POINTER(ctypes.c_float))
+    iptr = ctypes.c_void_p(intensity.data_ptr()) if intensity is not None else None
+    if on_gpu:
+        opts.stream = _stream_ptr(stream)
+        with torch.cuda.device(field.device):
+            rc = lib.bb_propagate_ex(ctypes.c_void_p(field.data_ptr()), ctypes.c_void_p(dn.data_ptr()), Nx, Ny, Nz,
+                                     dx, dz, lam, n0, iptr, ctypes.byref(opts))
+    else:
+        rc = lib.bb_propagate_host(ctypes.c_void_p(field.data_ptr()), ctypes.c_void_p(dn.data_ptr()), Nx, Ny, Nz,
+                                   dx, dz, lam, n0, iptr, ctypes.byref(opts))
+    _check(rc)
+    return field, intensity
+
+
+def propagate_simple(field: torch.Tensor, dn: torch.Tensor, dx, dz, lam, n0, intensity=None):
+    """The flat ``bb_propagate`` entry point (B = 1, n_ref = n0, default stream)."""
+    lib = load()
+    B, Ny, Nx = _field_shape(field)
+    if B != 1:
+        raise TypeError("bb_propagate takes one field")
+    _f32(dn, "dn")
+    with torch.cuda.device(field.device):
+        rc = lib.bb_propagate(ctypes.c_void_p(field.data_ptr()), ctypes.c_void_p(dn.data_ptr()), Nx, Ny, dn.shape[0],
+                              dx, dz, lam, n0,
+                              ctypes.c_void_p(intensity.data_ptr()) if intensity is not None else None)
+    _check(rc)
+    return field, intensity
+
+
+def nref_from_dn(dn: torch.Tensor, n0: float, slab: int, stream=None) -> torch.Tensor:
+    lib = load()
+    _f32(dn, "dn")
+    Nz, Ny, Nx = dn.shape
+    out = (ctypes.c_float * Nz)()
+    with torch.cuda.device(dn.device):
+        _check(lib.bb_nref_from_dn(ctypes.c_void_p(dn.data_ptr()), Nx, Ny, Nz, n0, slab, out, _stream_ptr(stream)))
+    return torch.tensor(list(out), dtype=torch.float32)
+
+
+def multiplex_psf(pos: torch.Tensor, phase: Optional[torch.Tensor], amp: Optional[torch.Tensor], NA: float,
+                  Nx: int, Ny: int, dx: float, lam: float, out: Optional[torch.Tensor] = None, stream=None):
+    lib = load()
+    _f32(pos, "pos")
+    if pos.dim() != 2 or pos.shape[1] != 2:
+        raise TypeError("pos must be [M][2]")
+    M = pos.shape[0]
+    for t, n in ((phase, "phase"), (amp, "amp")):
+        if t is not None and (_f32(t, n).numel() != M):
+            raise TypeError("%s must have M elements" % n)
+    if out is None:
+        out = torch.empty((Ny, Nx), dtype=torch.complex64, device=pos.device)
+    p = lambda t: ctypes.c_void_p(t.data_ptr()) if t is not None else None
+    with torch.cuda.device(pos.device):
+        _check(lib.bb_multiplex_psf(p(pos), p(phase), p(amp), M, NA, Nx, Ny, dx, lam, p(out), _stream_ptr(stream)))
+    return out
+
+
+def fft2(field: torch.Tensor, sign: int = -1, stream=None) -> torch.Tensor:
+    lib = load()
+    B, Ny, Nx = _field_shape(field)
+    with torch.cuda.device(field.device):
+        _check(lib.bb_fft2(ctypes.c_void_p(field.data_ptr()), Nx, Ny, B, sign, _stream_ptr(stream)))
+    return field
+
+
+def propagator_table(Nx: int, Ny: int, dx: float, dz: float, lam: float, nref: float, device="cuda", stream=None):
+    lib = load()
+    out = torch.empty((Ny, Nx), dtype=torch.complex64, device=device)
+    with torch.cuda.device(out.device):
+        _check(lib.bb_propagator_table(Nx, Ny, dx, dz, lam, nref, ctypes.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+    return out
+
+
+def device_status():
+    _check(load().bb_device_status())
+
+
+def launch_count() -> int:
+    return int(load().bb_launch_count())
+
+
+def version() -> int:
+    return int(load().bb_version())
+
+
+def shutdown():
+    load().bb_shutdown()

@@ -1,0 +1,73 @@
+"""Builds ``libbiobeam_b200.so`` in-tree with nvcc for sm_100a (no GPU needed to compile).
+
+``python -m paper_1706_02261_b200.build [--force]`` or :func:`build_library`.  The kernels
+are instantiated per line length (``bb_inst.cu`` compiled once per TX = Nx/32); the objects
+are compiled in parallel and linked into one shared library next to this file.
+"""
+from __future__ import annotations
+
+import concurrent.futures
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "_build")
+LIB = os.path.join(HERE, "libbiobeam_b200.so")
+INCLUDE = os.path.join(os.path.dirname(HERE), "include")
+TXS = (1, 2, 4, 8, 16, 32)
+
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+              "-Xcompiler", "-fPIC", "-I", INCLUDE]
+
+
+def _nvcc() -> str:
+    cand = os.path.join(os.environ.get("CUDA_HOME", "/usr/local/cuda"), "bin", "nvcc")
+    return cand if os.path.exists(cand) else "nvcc"
+
+
+def _sources():
+    deps = [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC))] + [os.path.join(INCLUDE, "bb.h")]
+    return deps
+
+
+def _stale(target: str, deps) -> bool:
+    if not os.path.exists(target):
+        return True
+    t = os.path.getmtime(target)
+    return any(os.path.getmtime(d) > t for d in deps)
+
+
+def _run(cmd):
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("command failed: %s\n%s\n%s" % (" ".join(cmd), r.stdout, r.stderr))
+    return r.stdout + r.stderr
+
+
+def build_library(force: bool = False, verbose: bool = False) -> str:
+    deps = _sources()
+    if not force and not _stale(LIB, deps):
+        return LIB
+    os.makedirs(OBJ, exist_ok=True)
+    nvcc = _nvcc()
+    jobs = []
+    for tx in TXS:
+        obj = os.path.join(OBJ, "bb_inst_tx%d.o" % tx)
+        jobs.append((obj, [nvcc, *NVCC_FLAGS, "-DBB_TX=%d" % tx, "-c", os.path.join(CSRC, "bb_inst.cu"), "-o", obj]))
+    obj_api = os.path.join(OBJ, "bb_api.o")
+    jobs.append((obj_api, [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, "bb_api.cu"), "-o", obj_api]))
+    todo = [(o, c) for o, c in jobs if force or _stale(o, deps)]
+    with concurrent.futures.ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
+        for out in ex.map(lambda oc: _run(oc[1]), todo):
+            if verbose and out.strip():
+                print(out)
+    tmp = LIB + ".tmp%d" % os.getpid()
+    _run([nvcc, "-shared", "-o", tmp, *[o for o, _ in jobs], "-lcudart_static", "-ldl", "-lrt", "-lpthread"])
+    os.replace(tmp, LIB)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build_library(force="--force" in sys.argv, verbose=True))

@@ -1,0 +1,635 @@
+// bb_api.cu -- C ABI of libbiobeam_b200.so (include/bb.h): argument checks, plan cache
+// (twiddle tables, propagator tables, workspace), launch sequencing.  All arithmetic of the
+// method runs in the kernels of bb_kernels.cuh / bb_aux_kernels.cuh.
+#include "../../include/bb.h"
+#include "bb_launch.h"
+#include "bb_aux_kernels.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <mutex>
+#include <string>
+#include <vector>
+
+namespace {
+
+using bb::KParams;
+typedef float2 cf;
+
+thread_local std::string g_err;
+std::mutex g_mu;
+unsigned long long g_launches = 0;
+
+int fail(int code, const char *fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_err = buf;
+    return code;
+}
+
+#define BB_CUDA(call)                                                                         \
+    do {                                                                                      \
+        cudaError_t e_ = (call);                                                              \
+        if (e_ != cudaSuccess)                                                                \
+            return fail(e_ == cudaErrorMemoryAllocation ? BB_ERR_OOM : BB_ERR_CUDA,           \
+                        "%s failed: %s", #call, cudaGetErrorString(e_));                      \
+    } while (0)
+
+const double kTwoPi = 6.283185307179586476925286766559;
+
+int log2_exact(int n) {
+    if (n <= 0 || (n & (n - 1))) return -1;
+    int l = 0;
+    while ((1 << l) < n) ++l;
+    return l;
+}
+
+// ------------------------------------------------------------------------------------------
+// Plan: everything cached for one (device, Nx, Ny).
+// ------------------------------------------------------------------------------------------
+struct TableKey {
+    float dx, dz, lambda, nref;
+    bool operator==(const TableKey &o) const {
+        return memcmp(this, &o, sizeof(TableKey)) == 0;
+    }
+};
+struct TableEntry { TableKey key; cf *ptr; unsigned long long last_use; };
+
+struct Plan {
+    int device, Nx, Ny;
+    cf *twx = nullptr, *twy = nullptr;
+    unsigned *bar = nullptr;
+    int *status = nullptr;
+    std::vector<TableEntry> tables;
+    size_t table_capacity = 0;
+    const cf **d_htab = nullptr;   // per-step arrays
+    float *d_phase = nullptr;
+    int step_cap = 0;
+    int grid = 0;                  // persistent grid size (<= SM count)
+    int sm_count = 0;
+    unsigned long long tick = 0;
+};
+
+std::vector<Plan *> g_plans;
+struct Workspace { void *ptr = nullptr; size_t bytes = 0; };
+Workspace g_ws_field, g_ws_dn, g_ws_I, g_ws_misc;
+
+int check_arch(int *device_out, int *sm_count) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(BB_ERR_CUDA, "cudaGetDevice failed: %s", cudaGetErrorString(e));
+    int major = 0, sms = 0;
+    BB_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    BB_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    if (major != 10)
+        return fail(BB_ERR_ARCH, "device %d has compute capability %d.x; this library is sm_100a only", dev, major);
+    *device_out = dev;
+    *sm_count = sms;
+    return BB_OK;
+}
+
+std::vector<cf> make_twiddles(int N) {
+    // tw[k1*T + t] = exp(-2 pi i k1 t / N), k1 < 32, t < T = N/32, from double
+    int T = N / 32;
+    std::vector<cf> tw((size_t)32 * T);
+    for (int k1 = 0; k1 < 32; ++k1)
+        for (int t = 0; t < T; ++t) {
+            double ph = -kTwoPi * (double)((long long)k1 * t) / (double)N;
+            tw[(size_t)k1 * T + t] = make_float2((float)cos(ph), (float)sin(ph));
+        }
+    return tw;
+}
+
+size_t table_budget_bytes() {
+    const char *e = getenv("BB_TABLE_CACHE_MB");
+    size_t mb = e ? (size_t)atoll(e) : 1024;
+    if (mb < 16) mb = 16;
+    return mb << 20;
+}
+
+int get_plan(int Nx, int Ny, Plan **out) {
+    int dev, sms;
+    int rc = check_arch(&dev, &sms);
+    if (rc) return rc;
+    for (Plan *p : g_plans)
+        if (p->device == dev && p->Nx == Nx && p->Ny == Ny) { *out = p; return BB_OK; }
+    Plan *p = new Plan();
+    p->device = dev; p->Nx = Nx; p->Ny = Ny; p->sm_count = sms;
+    std::vector<cf> tx = make_twiddles(Nx), ty = make_twiddles(Ny);
+    BB_CUDA(cudaMalloc(&p->twx, tx.size() * sizeof(cf)));
+    BB_CUDA(cudaMalloc(&p->twy, ty.size() * sizeof(cf)));
+    BB_CUDA(cudaMemcpy(p->twx, tx.data(), tx.size() * sizeof(cf), cudaMemcpyHostToDevice));
+    BB_CUDA(cudaMemcpy(p->twy, ty.data(), ty.size() * sizeof(cf), cudaMemcpyHostToDevice));
+    BB_CUDA(cudaMalloc(&p->bar, 256));
+    BB_CUDA(cudaMalloc(&p->status, 256));
+    BB_CUDA(cudaMemset(p->bar, 0, 256));
+    BB_CUDA(cudaMemset(p->status, 0, 256));
+    size_t tb = (size_t)Nx * Ny * sizeof(cf);
+    p->table_capacity = std::max<size_t>(2, std::min<size_t>(4096, table_budget_bytes() / tb));
+    rc = bb::kernel_prepare(Nx, Ny);
+    if (rc != 0) { delete p; return fail(BB_ERR_CUDA, "kernel_prepare failed: %s", cudaGetErrorString((cudaError_t)rc)); }
+    int per_sm = bb::kernel_blocks_per_sm(Nx, Ny);
+    if (per_sm < 1) { delete p; return fail(BB_ERR_CUDA, "BPM kernel does not fit on an SM"); }
+    p->grid = sms;
+    g_plans.push_back(p);
+    *out = p;
+    return BB_OK;
+}
+
+int ensure_steps(Plan *p, int Nz) {
+    if (Nz <= p->step_cap) return BB_OK;
+    if (p->d_htab) { cudaFree((void *)p->d_htab); cudaFree(p->d_phase); p->d_htab = nullptr; p->d_phase = nullptr; }
+    int cap = std::max(Nz, 1024);
+    BB_CUDA(cudaMalloc((void **)&p->d_htab, (size_t)cap * sizeof(cf *)));
+    BB_CUDA(cudaMalloc(&p->d_phase, (size_t)cap * sizeof(float)));
+    p->step_cap = cap;
+    return BB_OK;
+}
+
+int build_table(Plan *p, const TableKey &k, cf *dst, cudaStream_t s) {
+    double k0 = kTwoPi / (double)k.lambda;
+    double kk = k0 * (double)k.nref;
+    dim3 block(128), grid((p->Nx + 127) / 128, p->Ny);
+    bb::propagator_table_kernel<<<grid, block, 0, s>>>(dst, p->Nx, p->Ny, (double)k.dx, (double)k.dz, kk,
+                                                       1.0 / ((double)p->Nx * (double)p->Ny));
+    ++g_launches;
+    BB_CUDA(cudaGetLastError());
+    return BB_OK;
+}
+
+constexpr int kTableCacheFull = -1;   // internal: every cached table belongs to the launch being assembled
+
+// Returns the cached table for `k`, building it on `s` if needed.  Entries used at
+// tick >= protect_tick are never recycled (they belong to the launch being assembled).
+int get_table(Plan *p, const TableKey &k, cudaStream_t s, unsigned long long protect_tick, cf **out) {
+    for (TableEntry &e : p->tables)
+        if (e.key == k) { e.last_use = p->tick; *out = e.ptr; return BB_OK; }
+    TableEntry *slot = nullptr;
+    if (p->tables.size() < p->table_capacity) {
+        TableEntry e;
+        e.ptr = nullptr;
+        cudaError_t ce = cudaMalloc(&e.ptr, (size_t)p->Nx * p->Ny * sizeof(cf));
+        if (ce == cudaSuccess) { p->tables.push_back(e); slot = &p->tables.back(); }
+        else (void)cudaGetLastError();
+    }
+    if (!slot) {
+        for (TableEntry &e : p->tables)
+            if (e.last_use < protect_tick && (!slot || e.last_use < slot->last_use)) slot = &e;
+        if (!slot) return kTableCacheFull;
+    }
+    slot->key = k;
+    slot->last_use = p->tick;
+    int rc = build_table(p, k, slot->ptr, s);
+    if (rc) return rc;
+    *out = slot->ptr;
+    return BB_OK;
+}
+
+int validate_common(const void *field, const float *dn, int Nx, int Ny, int Nz, float dx, float dz,
+                    float lambda, float n0, const bb_opts *opts, int *B, unsigned *flags) {
+    if (!field) return fail(BB_ERR_INVALID_ARG, "field is NULL");
+    if (!dn) return fail(BB_ERR_INVALID_ARG, "dn_volume is NULL");
+    if (Nz < 1) return fail(BB_ERR_INVALID_ARG, "Nz = %d must be >= 1", Nz);
+    if (!(dx > 0.f) || !(dz > 0.f) || !(lambda > 0.f) || !(n0 > 0.f) || !std::isfinite(dx) ||
+        !std::isfinite(dz) || !std::isfinite(lambda) || !std::isfinite(n0))
+        return fail(BB_ERR_INVALID_ARG, "dx, dz, lambda, n0 must be positive and finite");
+    int lx = log2_exact(Nx), ly = log2_exact(Ny);
+    if (lx < 5 || lx > 10 || ly < 5 || ly > 10)
+        return fail(BB_ERR_UNSUPPORTED_SHAPE, "Nx = %d, Ny = %d: both must be powers of two in [32, 1024]", Nx, Ny);
+    *B = 1;
+    *flags = 0;
+    if (opts) {
+        if (opts->struct_size != (int)sizeof(bb_opts))
+            return fail(BB_ERR_INVALID_ARG, "bb_opts.struct_size = %d, expected %d", opts->struct_size, (int)sizeof(bb_opts));
+        if (opts->batch < 1) return fail(BB_ERR_INVALID_ARG, "batch = %d must be >= 1", opts->batch);
+        if (opts->flags & ~(BB_ACCUMULATE | BB_INTENSITY_PER_FIELD | BB_LAUNCH_PER_PHASE))
+            return fail(BB_ERR_INVALID_ARG, "unknown flag bits 0x%x", opts->flags);
+        if (opts->nref)
+            for (int j = 0; j < Nz; ++j)
+                if (!(opts->nref[j] > 0.f) || !std::isfinite(opts->nref[j]))
+                    return fail(BB_ERR_INVALID_ARG, "nref[%d] must be positive and finite", j);
+        *B = opts->batch;
+        *flags = opts->flags;
+    }
+    return BB_OK;
+}
+
+int batch_warps(int B) {
+    int bw = 1;
+    while (bw < B && bw < bb::kWarps) bw <<= 1;
+    return bw;
+}
+
+// Enqueue steps [j0, j1) of a propagation of Nz_total steps.  dn / inten point at slice j0.
+// Tables and per-step arrays for [j0, j1) must already be in place.
+int launch_steps(Plan *p, cf *field, const float *dn, float *inten, long long inten_bstride, int B,
+                 int Nz_total, int j0, int j1, float phase_b, unsigned flags, cudaStream_t s) {
+    KParams P;
+    memset(&P, 0, sizeof P);
+    P.field = field; P.dn = dn; P.inten = inten; P.inten_bstride = inten_bstride;
+    P.htab = p->d_htab; P.phase_a = p->d_phase; P.phase_b = phase_b;
+    P.Nx = p->Nx; P.Ny = p->Ny; P.B = B; P.BW = batch_warps(B);
+    P.Nz_total = Nz_total; P.j_base = j0;
+    P.mode = 0;
+    P.twx = p->twx; P.twy = p->twy; P.bar = p->bar; P.status = p->status;
+    P.flags = flags & 3u;
+    int p0 = (j0 == 0) ? 0 : 2 * j0 + 1, p1 = 2 * j1 + 1;
+    if (flags & BB_LAUNCH_PER_PHASE) {
+        for (int ph = p0; ph < p1; ++ph) {
+            P.p0 = ph; P.p1 = ph + 1;
+            cudaError_t e = bb::kernel_launch(p->Nx, p->Ny, P, p->grid, false, s);
+            ++g_launches;
+            if (e != cudaSuccess) return fail(BB_ERR_CUDA, "phase launch failed: %s", cudaGetErrorString(e));
+        }
+    } else {
+        P.p0 = p0; P.p1 = p1;
+        BB_CUDA(cudaMemsetAsync(p->bar, 0, sizeof(unsigned), s));
+        cudaError_t e = bb::kernel_launch(p->Nx, p->Ny, P, p->grid, true, s);
+        ++g_launches;
+        if (e != cudaSuccess) return fail(BB_ERR_CUDA, "cooperative launch failed: %s", cudaGetErrorString(e));
+    }
+    return BB_OK;
+}
+
+// Per-step tables and phase offsets for steps [j0, *j_done): the longest prefix of [j0, Nz)
+// whose distinct propagator tables fit the cache together (normally all of it).
+int prepare_steps(Plan *p, int Nz, int j0, float dx, float dz, float lambda, float n0, const float *nref,
+                  cudaStream_t s, std::vector<const cf *> &h_tab, std::vector<float> &h_phase, int *j_done) {
+    double k0 = kTwoPi / (double)lambda;
+    unsigned long long protect = ++p->tick;
+    const cf *last_ptr = nullptr;
+    float last_nref = 0.f;
+    int j = j0;
+    for (; j < Nz; ++j) {
+        float nr = nref ? nref[j] : n0;
+        if (!(last_ptr && nr == last_nref)) {
+            TableKey key = {dx, dz, lambda, nr};
+            cf *ptr = nullptr;
+            int rc = get_table(p, key, s, protect, &ptr);
+            if (rc == kTableCacheFull) break;                 // the rest goes into the next launch
+            if (rc) return rc;
+            last_ptr = ptr; last_nref = nr;
+        }
+        h_tab[j] = last_ptr;
+        h_phase[j] = (float)(k0 * (double)dz * ((double)n0 - (double)nr));
+    }
+    *j_done = j;
+    if (j == j0) return BB_OK;
+    int rc = ensure_steps(p, Nz);
+    if (rc) return rc;
+    BB_CUDA(cudaMemcpyAsync((void *)(p->d_htab + j0), h_tab.data() + j0, (size_t)(j - j0) * sizeof(cf *),
+                            cudaMemcpyHostToDevice, s));
+    BB_CUDA(cudaMemcpyAsync(p->d_phase + j0, h_phase.data() + j0, (size_t)(j - j0) * sizeof(float),
+                            cudaMemcpyHostToDevice, s));
+    return BB_OK;
+}
+
+int ws_reserve(Workspace &w, size_t bytes) {
+    if (bytes <= w.bytes) return BB_OK;
+    if (w.ptr) { cudaFree(w.ptr); w.ptr = nullptr; w.bytes = 0; }
+    BB_CUDA(cudaMalloc(&w.ptr, bytes));
+    w.bytes = bytes;
+    return BB_OK;
+}
+
+int run_program(Plan *p, cf *field, int B, const bb::PhaseProg *prog, int nprog, cudaStream_t s) {
+    KParams P;
+    memset(&P, 0, sizeof P);
+    P.field = field; P.Nx = p->Nx; P.Ny = p->Ny; P.B = B; P.BW = batch_warps(B);
+    P.mode = 1;
+    for (int i = 0; i < nprog; ++i) P.prog[i] = prog[i];
+    P.twx = p->twx; P.twy = p->twy; P.bar = p->bar; P.status = p->status;
+    P.p0 = 0; P.p1 = nprog;
+    BB_CUDA(cudaMemsetAsync(p->bar, 0, sizeof(unsigned), s));
+    cudaError_t e = bb::kernel_launch(p->Nx, p->Ny, P, p->grid, true, s);
+    ++g_launches;
+    if (e != cudaSuccess) return fail(BB_ERR_CUDA, "cooperative launch failed: %s", cudaGetErrorString(e));
+    return BB_OK;
+}
+
+}  // namespace
+
+namespace bb {
+#define BB_SWITCH_TX(fn, ...)                         \
+    switch (Nx / 32) {                                \
+        case 1: return inst1_##fn(__VA_ARGS__);       \
+        case 2: return inst2_##fn(__VA_ARGS__);       \
+        case 4: return inst4_##fn(__VA_ARGS__);       \
+        case 8: return inst8_##fn(__VA_ARGS__);       \
+        case 16: return inst16_##fn(__VA_ARGS__);     \
+        case 32: return inst32_##fn(__VA_ARGS__);     \
+    }
+int kernel_prepare(int Nx, int Ny) {
+    BB_SWITCH_TX(prepare, Ny / 32)
+    return (int)cudaErrorInvalidValue;
+}
+int kernel_blocks_per_sm(int Nx, int Ny) {
+    BB_SWITCH_TX(blocks_per_sm, Ny / 32)
+    return 0;
+}
+cudaError_t kernel_launch(int Nx, int Ny, const KParams &P, int grid, bool coop, cudaStream_t s) {
+    BB_SWITCH_TX(launch, Ny / 32, P, grid, coop, s)
+    return cudaErrorInvalidValue;
+}
+}  // namespace bb
+
+// ==========================================================================================
+extern "C" {
+
+const char *bb_last_error(void) { return g_err.c_str(); }
+int bb_version(void) { return 100; }
+unsigned long long bb_launch_count(void) { return g_launches; }
+
+void bb_shutdown(void) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    cudaDeviceSynchronize();
+    for (Plan *p : g_plans) {
+        cudaFree(p->twx); cudaFree(p->twy); cudaFree(p->bar); cudaFree(p->status);
+        for (TableEntry &e : p->tables) cudaFree(e.ptr);
+        if (p->d_htab) cudaFree((void *)p->d_htab);
+        if (p->d_phase) cudaFree(p->d_phase);
+        delete p;
+    }
+    g_plans.clear();
+    for (Workspace *w : {&g_ws_field, &g_ws_dn, &g_ws_I, &g_ws_misc}) {
+        if (w->ptr) cudaFree(w->ptr);
+        w->ptr = nullptr; w->bytes = 0;
+    }
+}
+
+int bb_device_status(void) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) return fail(BB_ERR_CUDA, "cudaDeviceSynchronize: %s", cudaGetErrorString(e));
+    for (Plan *p : g_plans) {
+        int st = 0;
+        BB_CUDA(cudaMemcpy(&st, p->status, sizeof st, cudaMemcpyDeviceToHost));
+        if (st != 0) {
+            cudaMemset(p->status, 0, sizeof st);
+            return fail(BB_ERR_INTERNAL, "grid barrier watchdog tripped (Nx=%d, Ny=%d)", p->Nx, p->Ny);
+        }
+    }
+    return BB_OK;
+}
+
+int bb_propagate_ex(void *field, const float *dn, int Nx, int Ny, int Nz, float dx, float dz, float lambda,
+                    float n0, float *intensity_out, const bb_opts *opts) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    int B; unsigned flags;
+    int rc = validate_common(field, dn, Nx, Ny, Nz, dx, dz, lambda, n0, opts, &B, &flags);
+    if (rc) return rc;
+    Plan *p;
+    rc = get_plan(Nx, Ny, &p);
+    if (rc) return rc;
+    cudaStream_t s = opts ? (cudaStream_t)opts->stream : (cudaStream_t)0;
+    const float *nref = opts ? opts->nref : nullptr;
+    std::vector<const cf *> h_tab(Nz);
+    std::vector<float> h_phase(Nz);
+    double k0 = kTwoPi / (double)lambda;
+    float phase_b = (float)(k0 * (double)dz);
+    size_t npx = (size_t)Nx * Ny;
+    int j0 = 0;
+    while (j0 < Nz) {
+        int j1;
+        rc = prepare_steps(p, Nz, j0, dx, dz, lambda, n0, nref, s, h_tab, h_phase, &j1);
+        if (rc) return rc;
+        if (j1 <= j0) return fail(BB_ERR_OOM, "propagator table cache too small for one step");
+        rc = launch_steps(p, (cf *)field, dn + (size_t)j0 * npx,
+                          intensity_out ? intensity_out + (size_t)j0 * npx : nullptr,
+                          (long long)Nz * (long long)npx, B, Nz, j0, j1, phase_b, flags, s);
+        if (rc) return rc;
+        j0 = j1;
+    }
+    return BB_OK;
+}
+
+int bb_propagate(void *field, const float *dn, int Nx, int Ny, int Nz, float dx, float dz, float lambda,
+                 float n0, float *intensity_out) {
+    return bb_propagate_ex(field, dn, Nx, Ny, Nz, dx, dz, lambda, n0, intensity_out, nullptr);
+}
+
+int bb_propagate_host(void *field_host, const float *dn_host, int Nx, int Ny, int Nz, float dx, float dz,
+                      float lambda, float n0, float *inten_host, const bb_opts *opts) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    int B; unsigned flags;
+    int rc = validate_common(field_host, dn_host, Nx, Ny, Nz, dx, dz, lambda, n0, opts, &B, &flags);
+    if (rc) return rc;
+    Plan *p;
+    rc = get_plan(Nx, Ny, &p);
+    if (rc) return rc;
+    const float *nref = opts ? opts->nref : nullptr;
+    const size_t npx = (size_t)Nx * Ny;
+    const bool per_field = (flags & BB_INTENSITY_PER_FIELD) != 0;
+    const int IB = per_field ? B : 1;                        // intensity volumes
+    // z-chunks of ~32 MiB of dn, three buffers in flight per direction
+    const int NBUF = 3;
+    int CZ = (int)std::max<size_t>(1, ((size_t)32 << 20) / (npx * sizeof(float)));
+    CZ = std::min(CZ, Nz);
+    rc = ws_reserve(g_ws_field, (size_t)B * npx * sizeof(cf));
+    if (!rc) rc = ws_reserve(g_ws_dn, (size_t)NBUF * CZ * npx * sizeof(float));
+    if (!rc && inten_host) rc = ws_reserve(g_ws_I, (size_t)NBUF * IB * CZ * npx * sizeof(float));
+    if (rc) return rc;
+    cf *d_field = (cf *)g_ws_field.ptr;
+    float *d_dn = (float *)g_ws_dn.ptr;
+    float *d_I = inten_host ? (float *)g_ws_I.ptr : nullptr;
+
+    cudaStream_t s_in, s_run, s_out;
+    BB_CUDA(cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking));
+    BB_CUDA(cudaStreamCreateWithFlags(&s_run, cudaStreamNonBlocking));
+    BB_CUDA(cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking));
+    const int nchunks = (Nz + CZ - 1) / CZ;
+    std::vector<cudaEvent_t> ev_in(nchunks), ev_run(nchunks), ev_out(nchunks);
+    for (int c = 0; c < nchunks; ++c) {
+        cudaEventCreateWithFlags(&ev_in[c], cudaEventDisableTiming);
+        cudaEventCreateWithFlags(&ev_run[c], cudaEventDisableTiming);
+        cudaEventCreateWithFlags(&ev_out[c], cudaEventDisableTiming);
+    }
+    int result = BB_OK;
+    auto cleanup = [&]() {
+        cudaStreamSynchronize(s_in); cudaStreamSynchronize(s_run); cudaStreamSynchronize(s_out);
+        for (int c = 0; c < nchunks; ++c) { cudaEventDestroy(ev_in[c]); cudaEventDestroy(ev_run[c]); cudaEventDestroy(ev_out[c]); }
+        cudaStreamDestroy(s_in); cudaStreamDestroy(s_run); cudaStreamDestroy(s_out);
+    };
+#define BB_TRY(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { result = fail(BB_ERR_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_)); cleanup(); return result; } } while (0)
+
+    BB_TRY(cudaMemcpyAsync(d_field, field_host, (size_t)B * npx * sizeof(cf), cudaMemcpyHostToDevice, s_run));
+    std::vector<const cf *> h_tab(Nz);
+    std::vector<float> h_phase(Nz);
+    double k0 = kTwoPi / (double)lambda;
+    float phase_b = (float)(k0 * (double)dz);
+    int prepared = 0;                                        // steps [0, prepared) have tables in place
+    for (int c = 0; c < nchunks; ++c) {
+        const int j0 = c * CZ, j1 = std::min(Nz, j0 + CZ), nz = j1 - j0;
+        const int buf = c % NBUF;
+        float *dn_b = d_dn + (size_t)buf * CZ * npx;
+        float *I_b = d_I ? d_I + (size_t)buf * IB * CZ * npx : nullptr;
+        // dn chunk in: the buffer is free once the chunk that last used it has been computed
+        if (c >= NBUF) BB_TRY(cudaStreamWaitEvent(s_in, ev_run[c - NBUF], 0));
+        BB_TRY(cudaMemcpyAsync(dn_b, dn_host + (size_t)j0 * npx, (size_t)nz * npx * sizeof(float),
+                               cudaMemcpyHostToDevice, s_in));
+        BB_TRY(cudaEventRecord(ev_in[c], s_in));
+        BB_TRY(cudaStreamWaitEvent(s_run, ev_in[c], 0));
+        if (I_b && c >= NBUF) BB_TRY(cudaStreamWaitEvent(s_run, ev_out[c - NBUF], 0));
+        if (I_b && (flags & BB_ACCUMULATE)) {                // existing contents are part of the input
+            for (int b = 0; b < IB; ++b)
+                BB_TRY(cudaMemcpyAsync(I_b + (size_t)b * CZ * npx, inten_host + ((size_t)b * Nz + j0) * npx,
+                                       (size_t)nz * npx * sizeof(float), cudaMemcpyHostToDevice, s_run));
+        }
+        int ja = j0;
+        while (ja < j1) {
+            if (ja >= prepared) {
+                rc = prepare_steps(p, Nz, ja, dx, dz, lambda, n0, nref, s_run, h_tab, h_phase, &prepared);
+                if (rc || prepared <= ja) { cleanup(); return rc ? rc : fail(BB_ERR_OOM, "propagator table cache too small"); }
+            }
+            int jb = std::min(j1, prepared);
+            rc = launch_steps(p, d_field, dn_b + (size_t)(ja - j0) * npx,
+                              I_b ? I_b + (size_t)(ja - j0) * npx : nullptr, (long long)CZ * (long long)npx,
+                              B, Nz, ja, jb, phase_b, flags, s_run);
+            if (rc) { cleanup(); return rc; }
+            ja = jb;
+        }
+        BB_TRY(cudaEventRecord(ev_run[c], s_run));
+        if (I_b) {
+            BB_TRY(cudaStreamWaitEvent(s_out, ev_run[c], 0));
+            for (int b = 0; b < IB; ++b)
+                BB_TRY(cudaMemcpyAsync(inten_host + ((size_t)b * Nz + j0) * npx, I_b + (size_t)b * CZ * npx,
+                                       (size_t)nz * npx * sizeof(float), cudaMemcpyDeviceToHost, s_out));
+            BB_TRY(cudaEventRecord(ev_out[c], s_out));
+        }
+    }
+    BB_TRY(cudaMemcpyAsync(field_host, d_field, (size_t)B * npx * sizeof(cf), cudaMemcpyDeviceToHost, s_run));
+    BB_TRY(cudaStreamSynchronize(s_run));
+    BB_TRY(cudaStreamSynchronize(s_out));
+    BB_TRY(cudaStreamSynchronize(s_in));
+    int st = 0;
+    BB_TRY(cudaMemcpy(&st, p->status, sizeof st, cudaMemcpyDeviceToHost));
+    cleanup();
+#undef BB_TRY
+    if (st != 0) {
+        cudaMemset(p->status, 0, sizeof st);
+        return fail(BB_ERR_INTERNAL, "grid barrier watchdog tripped");
+    }
+    return result;
+}
+
+int bb_nref_from_dn(const float *dn, int Nx, int Ny, int Nz, float n0, int slab, float *nref_out, void *stream) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!dn || !nref_out) return fail(BB_ERR_INVALID_ARG, "dn_volume or nref_out is NULL");
+    if (Nx < 1 || Ny < 1 || Nz < 1 || slab < 1) return fail(BB_ERR_INVALID_ARG, "Nx, Ny, Nz, slab must be >= 1");
+    int dev, sms;
+    int rc = check_arch(&dev, &sms);
+    if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    const int NP = 16;
+    rc = ws_reserve(g_ws_misc, (size_t)Nz * NP * sizeof(double));
+    if (rc) return rc;
+    double *d_part = (double *)g_ws_misc.ptr;
+    size_t npx = (size_t)Nx * Ny;
+    for (int j0 = 0; j0 < Nz; j0 += 32768) {                 // gridDim.y limit
+        int nz = std::min(32768, Nz - j0);
+        bb::slice_sum_kernel<<<dim3(NP, nz), 256, 0, s>>>(dn + (size_t)j0 * npx, npx, d_part + (size_t)j0 * NP);
+        ++g_launches;
+    }
+    BB_CUDA(cudaGetLastError());
+    std::vector<double> part((size_t)Nz * NP);
+    BB_CUDA(cudaMemcpyAsync(part.data(), d_part, part.size() * sizeof(double), cudaMemcpyDeviceToHost, s));
+    BB_CUDA(cudaStreamSynchronize(s));
+    for (int j0 = 0; j0 < Nz; j0 += slab) {
+        int j1 = std::min(Nz, j0 + slab);
+        long double sum = 0.0L;
+        for (int j = j0; j < j1; ++j) {
+            double sj = 0.0;
+            for (int q = 0; q < NP; ++q) sj += part[(size_t)j * NP + q];
+            sum += sj;
+        }
+        double mean = (double)(sum / ((long double)npx * (long double)(j1 - j0)));
+        float v = (float)((double)n0 + mean);
+        for (int j = j0; j < j1; ++j) nref_out[j] = v;
+    }
+    return BB_OK;
+}
+
+int bb_fft2(void *field, int Nx, int Ny, int batch, int sign, void *stream) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!field) return fail(BB_ERR_INVALID_ARG, "field is NULL");
+    if (batch < 1) return fail(BB_ERR_INVALID_ARG, "batch must be >= 1");
+    if (sign != -1 && sign != 1) return fail(BB_ERR_INVALID_ARG, "sign must be -1 or +1");
+    int lx = log2_exact(Nx), ly = log2_exact(Ny);
+    if (lx < 5 || lx > 10 || ly < 5 || ly > 10)
+        return fail(BB_ERR_UNSUPPORTED_SHAPE, "Nx = %d, Ny = %d: both must be powers of two in [32, 1024]", Nx, Ny);
+    Plan *p;
+    int rc = get_plan(Nx, Ny, &p);
+    if (rc) return rc;
+    bb::PhaseProg prog[2];
+    if (sign < 0) {
+        prog[0] = {1, 0, 1, 1.f};
+        prog[1] = {0, 0, 1, 1.f};
+    } else {
+        prog[0] = {0, 1, 0, 1.f};
+        prog[1] = {1, 1, 0, (float)(1.0 / ((double)Nx * (double)Ny))};
+    }
+    return run_program(p, (cf *)field, batch, prog, 2, (cudaStream_t)stream);
+}
+
+int bb_propagator_table(int Nx, int Ny, float dx, float dz, float lambda, float nref, void *out, void *stream) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!out) return fail(BB_ERR_INVALID_ARG, "table_out is NULL");
+    if (!(dx > 0.f) || !(dz > 0.f) || !(lambda > 0.f) || !(nref > 0.f))
+        return fail(BB_ERR_INVALID_ARG, "dx, dz, lambda, nref must be positive");
+    int lx = log2_exact(Nx), ly = log2_exact(Ny);
+    if (lx < 5 || lx > 10 || ly < 5 || ly > 10)
+        return fail(BB_ERR_UNSUPPORTED_SHAPE, "Nx = %d, Ny = %d: both must be powers of two in [32, 1024]", Nx, Ny);
+    Plan *p;
+    int rc = get_plan(Nx, Ny, &p);
+    if (rc) return rc;
+    TableKey k = {dx, dz, lambda, nref};
+    return build_table(p, k, (cf *)out, (cudaStream_t)stream);
+}
+
+int bb_multiplex_psf(const float *pos, const float *phase, const float *amp, int M, float NA, int Nx, int Ny,
+                     float dx, float lambda, void *field_out, void *stream) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!pos || !field_out) return fail(BB_ERR_INVALID_ARG, "emitter_positions or field_out is NULL");
+    if (M < 1) return fail(BB_ERR_INVALID_ARG, "M = %d must be >= 1", M);
+    if (!(NA > 0.f) || !(dx > 0.f) || !(lambda > 0.f) || !std::isfinite(NA))
+        return fail(BB_ERR_INVALID_ARG, "NA, dx, lambda must be positive and finite");
+    int lx = log2_exact(Nx), ly = log2_exact(Ny);
+    if (lx < 5 || lx > 10 || ly < 5 || ly > 10)
+        return fail(BB_ERR_UNSUPPORTED_SHAPE, "Nx = %d, Ny = %d: both must be powers of two in [32, 1024]", Nx, Ny);
+    Plan *p;
+    int rc = get_plan(Nx, Ny, &p);
+    if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    // pupil pixel count, in double, same expression as the kernel's inside test
+    const double ddx = dx, k0 = kTwoPi / (double)lambda, kc2 = (k0 * (double)NA) * (k0 * (double)NA);
+    long long count = 0;
+    std::vector<double> kx2(Nx), ky2(Ny);
+    for (int i = 0; i < Nx; ++i) { int f = (i < Nx / 2) ? i : i - Nx; double k = kTwoPi * (double)f / ((double)Nx * ddx); kx2[i] = k * k; }
+    for (int i = 0; i < Ny; ++i) { int f = (i < Ny / 2) ? i : i - Ny; double k = kTwoPi * (double)f / ((double)Ny * ddx); ky2[i] = k * k; }
+    for (int q = 0; q < Ny; ++q)
+        for (int i = 0; i < Nx; ++i)
+            if (kx2[i] + ky2[q] <= kc2) ++count;
+    if (count == 0) return fail(BB_ERR_INVALID_ARG, "pupil of NA = %g contains no grid frequency", (double)NA);
+    rc = ws_reserve(g_ws_misc, std::max<size_t>((size_t)M * sizeof(bb::EmitterPrep), 4096));
+    if (rc) return rc;
+    bb::EmitterPrep *em = (bb::EmitterPrep *)g_ws_misc.ptr;
+    bb::emitter_prep_kernel<<<(M + 127) / 128, 128, 0, s>>>(pos, phase, amp, M, Nx, Ny, ddx, em);
+    ++g_launches;
+    dim3 block(128), grid((Nx + 127) / 128, Ny);
+    bb::multiplex_spectrum_kernel<<<grid, block, 128 * sizeof(bb::EmitterPrep), s>>>((cf *)field_out, Nx, Ny, ddx, kc2, em, M);
+    ++g_launches;
+    BB_CUDA(cudaGetLastError());
+    bb::PhaseProg prog[2];
+    prog[0] = {0, 1, 0, 1.f};
+    prog[1] = {1, 1, 0, (float)(1.0 / (double)count)};
+    return run_program(p, (cf *)field_out, 1, prog, 2, s);
+}
+
+}  // extern "C"

@@ -1,0 +1,171 @@
+// bb_fft.cuh -- in-register complex64 line FFTs for sm_100a.
+//
+// A line of N = 32*T points is transformed by T threads holding 32 points each, as a
+// two-factor Cooley-Tukey split N = 32 x T:
+//     n = T*n1 + n2  (n1 < 32, n2 < T),   k = k1 + 32*k2  (k1 < 32, k2 < T)
+//     X[k1 + 32 k2] = sum_n2 [ w_N^(n2 k1) * ( sum_n1 x[T n1 + n2] w_32^(n1 k1) ) ] w_T^(n2 k2)
+// thread n2 computes the inner radix-32 DFT over its 32 registers, multiplies by the
+// twiddle w_N^(n2 k1) (fp64-built table, read from shared memory), the 32 x T matrix is
+// transposed through padded shared memory, and thread t then does 32/T radix-T DFTs over
+// n2 for k1 = t + T*m.  The result lands in the SAME distribution as the input
+// (thread t holds X[t + T*j], j < 32), so transform -> pointwise -> transform chains stay in
+// registers.  Radix kernels are fully unrolled radix-2 decimation-in-frequency recursions
+// with compile-time twiddles (correctly rounded from double).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace bb {
+
+typedef float2 cf;
+
+__device__ __forceinline__ cf cadd(cf a, cf b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ cf csub(cf a, cf b) { return make_float2(a.x - b.x, a.y - b.y); }
+// a * w
+__device__ __forceinline__ cf cmul(cf a, cf w) {
+    return make_float2(fmaf(a.x, w.x, -(a.y * w.y)), fmaf(a.x, w.y, a.y * w.x));
+}
+// a * conj(w)
+__device__ __forceinline__ cf cmulc(cf a, cf w) {
+    return make_float2(fmaf(a.x, w.x, a.y * w.y), fmaf(a.y, w.x, -(a.x * w.y)));
+}
+
+// cos(2 pi m / 32), m = 0..16, rounded from double at compile time.
+__device__ __forceinline__ constexpr float cos32(int m) {
+    constexpr double C[17] = {
+        1.0,
+        0.98078528040323044912618223613424,
+        0.92387953251128675612818318939679,
+        0.83146961230254523707878837761791,
+        0.70710678118654752440084436210485,
+        0.55557023301960222474283081394853,
+        0.38268343236508977172845998403040,
+        0.19509032201612826784828486847702,
+        0.0,
+        -0.19509032201612826784828486847702,
+        -0.38268343236508977172845998403040,
+        -0.55557023301960222474283081394853,
+        -0.70710678118654752440084436210485,
+        -0.83146961230254523707878837761791,
+        -0.92387953251128675612818318939679,
+        -0.98078528040323044912618223613424,
+        -1.0};
+    return (float)C[m];
+}
+__device__ __forceinline__ constexpr float sin32(int m) {   // sin(2 pi m/32) = cos(2 pi (m-8)/32), m in [0,16]
+    return cos32(m >= 8 ? m - 8 : 8 - m);
+}
+
+// a * exp(SIGN * 2 pi i * M / 32),  0 <= M < 16
+template <int M, int SIGN>
+__device__ __forceinline__ cf mul_w32(cf a) {
+    if constexpr (M == 0) {
+        return a;
+    } else if constexpr (M == 8) {              // * (SIGN i)
+        return SIGN < 0 ? make_float2(a.y, -a.x) : make_float2(-a.y, a.x);
+    } else if constexpr (M == 4) {              // * (1 + SIGN i)/sqrt2
+        constexpr float r = cos32(4);
+        return SIGN < 0 ? make_float2((a.x + a.y) * r, (a.y - a.x) * r)
+                        : make_float2((a.x - a.y) * r, (a.y + a.x) * r);
+    } else if constexpr (M == 12) {             // * (-1 + SIGN i)/sqrt2
+        constexpr float r = cos32(4);
+        return SIGN < 0 ? make_float2((a.y - a.x) * r, -(a.x + a.y) * r)
+                        : make_float2(-(a.x + a.y) * r, (a.x - a.y) * r);
+    } else {
+        constexpr float c = cos32(M);
+        constexpr float s = SIGN < 0 ? -sin32(M) : sin32(M);
+        return make_float2(fmaf(a.x, c, -(a.y * s)), fmaf(a.x, s, a.y * c));
+    }
+}
+
+// Radix-R DFT over registers, natural order in and out:
+//   v[k] <- sum_n v[n] exp(SIGN 2 pi i n k / R)
+template <int R, int SIGN>
+struct Dft {
+    static __device__ __forceinline__ void run(cf (&v)[R]) {
+        constexpr int H = R / 2;
+        cf a[H], b[H];
+#pragma unroll
+        for (int n = 0; n < H; ++n) {
+            a[n] = cadd(v[n], v[n + H]);
+            b[n] = csub(v[n], v[n + H]);
+        }
+        twiddle<0>(b);
+        Dft<H, SIGN>::run(a);
+        Dft<H, SIGN>::run(b);
+#pragma unroll
+        for (int k = 0; k < H; ++k) {
+            v[2 * k] = a[k];
+            v[2 * k + 1] = b[k];
+        }
+    }
+    template <int n>
+    static __device__ __forceinline__ void twiddle(cf (&b)[R / 2]) {
+        if constexpr (n < R / 2) {
+            b[n] = mul_w32<n*(32 / R), SIGN>(b[n]);
+            twiddle<n + 1>(b);
+        }
+    }
+};
+template <int SIGN>
+struct Dft<2, SIGN> {
+    static __device__ __forceinline__ void run(cf (&v)[2]) {
+        cf a = cadd(v[0], v[1]);
+        v[1] = csub(v[0], v[1]);
+        v[0] = a;
+    }
+};
+template <int SIGN>
+struct Dft<1, SIGN> {
+    static __device__ __forceinline__ void run(cf (&)[1]) {}
+};
+
+// Shared-memory geometry of the 32 x T transpose (float2 units); paddings found by brute
+// force to make both the stores and the loads bank-conflict free for 64-bit accesses.
+//   row mapping   : lane = g*T + t, one region per line g of a warp
+//   column mapping: r = c + CW*t inside a tile of CW columns, one region per column c
+template <int T> struct RowGeom {
+    static constexpr int S = T + 1;                                   // stride between k1 rows
+    static constexpr int RS = 32 * S + (T < 16 ? T : 0);              // stride between lines
+    static constexpr int WARP = T == 1 ? 0 : (32 / T) * RS;           // float2 per warp (T = 1: no transpose)
+};
+template <int T, int CW> struct ColGeom {
+    static constexpr int S = (CW == 16) ? T : T + 1;
+    static constexpr int RS = 32 * S + (CW == 16 ? 1 : (CW == 8 ? 2 : (T == 2 ? 2 : 4)));
+    static constexpr int TILE = T == 1 ? 0 : CW * RS;                 // float2 per tile slot
+};
+
+struct SyncWarp  { __device__ __forceinline__ void operator()() const { __syncwarp(); } };
+struct SyncBlock { __device__ __forceinline__ void operator()() const { __syncthreads(); } };
+
+// One line FFT (see file header).  v: this thread's 32 points x[t + T*j].
+//   tw   : shared, [32][T], tw[k1*T + t] = exp(-2 pi i k1 t / N)  (conjugated for SIGN = +1)
+//   ybuf : shared, base of this thread's line region; S = stride between k1 rows
+template <int T, int SIGN, int S, class Sync>
+__device__ __forceinline__ void line_fft(cf (&v)[32], const cf *__restrict__ tw, cf *ybuf, int t, Sync sync) {
+    Dft<32, SIGN>::run(v);
+    if constexpr (T > 1) {
+#pragma unroll
+        for (int k1 = 0; k1 < 32; ++k1) {
+            cf x = v[k1];
+            if (k1 > 0) {
+                cf w = tw[k1 * T + t];
+                x = SIGN < 0 ? cmul(x, w) : cmulc(x, w);
+            }
+            ybuf[k1 * S + t] = x;
+        }
+        sync();
+        constexpr int G = 32 / T;
+#pragma unroll
+        for (int m = 0; m < G; ++m) {
+            cf w[T];
+#pragma unroll
+            for (int n2 = 0; n2 < T; ++n2) w[n2] = ybuf[(t + T * m) * S + n2];
+            Dft<T, SIGN>::run(w);
+#pragma unroll
+            for (int k2 = 0; k2 < T; ++k2) v[m + G * k2] = w[k2];
+        }
+        sync();
+    }
+}
+
+}  // namespace bb

@@ -1,0 +1,26 @@
+// bb_launch.h -- host-side entry points of the per-shape kernel instantiations (bb_inst.cu is
+// compiled once per TX = Nx/32; each object holds the kernels for every TY = Ny/32).
+#pragma once
+#include "bb_kernels.cuh"
+
+namespace bb {
+
+// One set per TX in {1, 2, 4, 8, 16, 32}.
+#define BB_DECLARE_INST(TX)                                                                     \
+    cudaError_t inst##TX##_prepare(int TY);                                                     \
+    int inst##TX##_blocks_per_sm(int TY);                                                       \
+    cudaError_t inst##TX##_launch(int TY, const KParams &P, int grid, bool coop, cudaStream_t s);
+BB_DECLARE_INST(1)
+BB_DECLARE_INST(2)
+BB_DECLARE_INST(4)
+BB_DECLARE_INST(8)
+BB_DECLARE_INST(16)
+BB_DECLARE_INST(32)
+#undef BB_DECLARE_INST
+
+// Dispatch on (Nx, Ny); defined in bb_api.cu.
+int kernel_prepare(int Nx, int Ny);           // returns a cudaError_t value
+int kernel_blocks_per_sm(int Nx, int Ny);
+cudaError_t kernel_launch(int Nx, int Ny, const KParams &P, int grid, bool coop, cudaStream_t s);
+
+}  // namespace bb
