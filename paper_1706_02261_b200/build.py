@@ -64,7 +64,8 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
             if verbose and out.strip():
                 print(out)
     tmp = LIB + ".tmp%d" % os.getpid()
-    _run([nvcc, "-shared", "-o", tmp, *[o for o, _ in jobs], "-lcudart_static", "-ldl", "-lrt", "-lpthread"])
+    _run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp, *[o for o, _ in jobs],
+          "-lcudart_static", "-ldl", "-lrt", "-lpthread"])
     os.replace(tmp, LIB)
     return LIB
 

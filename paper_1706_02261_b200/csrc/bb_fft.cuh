@@ -29,8 +29,9 @@ __device__ __forceinline__ cf cmulc(cf a, cf w) {
     return make_float2(fmaf(a.x, w.x, a.y * w.y), fmaf(a.y, w.x, -(a.x * w.y)));
 }
 
-// cos(2 pi m / 32), m = 0..16, rounded from double at compile time.
-__device__ __forceinline__ constexpr float cos32(int m) {
+// cos(2 pi m / 32), m = 0..16, in double; the kernels use it as a two-float constant
+// hi = (float)c, lo = (float)(c - hi).
+__device__ __forceinline__ constexpr double cos32d(int m) {
     constexpr double C[17] = {
         1.0,
         0.98078528040323044912618223613424,
@@ -49,31 +50,44 @@ __device__ __forceinline__ constexpr float cos32(int m) {
         -0.92387953251128675612818318939679,
         -0.98078528040323044912618223613424,
         -1.0};
-    return (float)C[m];
+    return C[m];
 }
-__device__ __forceinline__ constexpr float sin32(int m) {   // sin(2 pi m/32) = cos(2 pi (m-8)/32), m in [0,16]
-    return cos32(m >= 8 ? m - 8 : 8 - m);
+__device__ __forceinline__ constexpr double sin32d(int m) {   // sin(2 pi m/32) = cos(2 pi (m-8)/32), m in [0,16]
+    return cos32d(m >= 8 ? m - 8 : 8 - m);
 }
+__device__ __forceinline__ constexpr float hi_of(double c) { return (float)c; }
+__device__ __forceinline__ constexpr float lo_of(double c) { return (float)(c - (double)(float)c); }
 
-// a * exp(SIGN * 2 pi i * M / 32),  0 <= M < 16
+// t * r for a two-float constant r = rh + rl: one rounding of t*rh + t*rl.
+__device__ __forceinline__ float mul_hilo(float t, float rh, float rl) { return fmaf(t, rh, t * rl); }
+
+// a * exp(SIGN * 2 pi i * M / 32),  0 <= M < 16.
+// The constants are two-float values and the low parts enter INSIDE the fused multiply-add
+// chain, so each product is an unbiased rounding of the exact one.  With plain float32
+// constants every 32nd root of unity happens to round to |w| < 1 (by 0.7e-8 .. 2.9e-8); the
+// same shrink factor would then hit the field at every step and the error of a propagation
+// would grow linearly with the number of steps.
 template <int M, int SIGN>
 __device__ __forceinline__ cf mul_w32(cf a) {
     if constexpr (M == 0) {
         return a;
     } else if constexpr (M == 8) {              // * (SIGN i)
         return SIGN < 0 ? make_float2(a.y, -a.x) : make_float2(-a.y, a.x);
-    } else if constexpr (M == 4) {              // * (1 + SIGN i)/sqrt2
-        constexpr float r = cos32(4);
-        return SIGN < 0 ? make_float2((a.x + a.y) * r, (a.y - a.x) * r)
-                        : make_float2((a.x - a.y) * r, (a.y + a.x) * r);
-    } else if constexpr (M == 12) {             // * (-1 + SIGN i)/sqrt2
-        constexpr float r = cos32(4);
-        return SIGN < 0 ? make_float2((a.y - a.x) * r, -(a.x + a.y) * r)
-                        : make_float2(-(a.x + a.y) * r, (a.x - a.y) * r);
+    } else if constexpr (M == 4 || M == 12) {   // * (+-1 + SIGN i)/sqrt2
+        constexpr float rh = hi_of(cos32d(4)), rl = lo_of(cos32d(4));
+        const float p = a.x + a.y, q = a.y - a.x;       // p = x + y, q = y - x
+        if constexpr (M == 4)
+            return SIGN < 0 ? make_float2(mul_hilo(p, rh, rl), mul_hilo(q, rh, rl))
+                            : make_float2(mul_hilo(-q, rh, rl), mul_hilo(p, rh, rl));
+        else
+            return SIGN < 0 ? make_float2(mul_hilo(q, rh, rl), mul_hilo(-p, rh, rl))
+                            : make_float2(mul_hilo(-p, rh, rl), mul_hilo(-q, rh, rl));
     } else {
-        constexpr float c = cos32(M);
-        constexpr float s = SIGN < 0 ? -sin32(M) : sin32(M);
-        return make_float2(fmaf(a.x, c, -(a.y * s)), fmaf(a.x, s, a.y * c));
+        constexpr double cd = cos32d(M), sd = SIGN < 0 ? -sin32d(M) : sin32d(M);
+        constexpr float c = hi_of(cd), cl = lo_of(cd), s = hi_of(sd), sl = lo_of(sd);
+        const float lre = fmaf(a.x, cl, -(a.y * sl));
+        const float lim = fmaf(a.x, sl, a.y * cl);
+        return make_float2(fmaf(a.x, c, fmaf(-a.y, s, lre)), fmaf(a.x, s, fmaf(a.y, c, lim)));
     }
 }
 

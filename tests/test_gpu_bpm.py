@@ -1,0 +1,229 @@
+"""-m gpu: end-to-end parity of the CUDA BPM (through the C ABI) with the oracle, element by
+element on the same seeded inputs (SURVEY section 4 tier T2, section 8c reading A16).
+
+Tolerance: BASELINE.json:north_star -- relative L2 <= 1e-4 on the final complex field and on
+the intensity volume (one ratio over the whole volume).  Small cases use a tighter bound
+proportional to their step count (~1e-7 per step)."""
+import numpy as np
+import pytest
+import torch
+
+from conftest import rel_l2
+from gpu_common import StreamCompare, gpu_inputs, need_gpu, oracle_field0
+from paper_1706_02261_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4
+
+
+def small_tol(nz):
+    return 2e-6 + 2.5e-7 * nz
+
+
+def run_both(bb, oracle, w, dn, f0, nref, flags=0, intensity_init=None):
+    """GPU result (final fields, intensity) and oracle result for the same inputs."""
+    B = f0.shape[0]
+    d = torch.from_numpy(f0).cuda()
+    per_field = bool(flags & bb.INTENSITY_PER_FIELD)
+    shape = ((B,) if per_field else ()) + tuple(dn.shape)
+    if intensity_init is None:
+        I = torch.full(shape, float("nan"), device="cuda")
+    else:
+        I = torch.from_numpy(intensity_init.astype(np.float32)).cuda()
+    bb.propagate(d, dn.cuda(), w.dx, w.dz, w.lam, w.n0, intensity=I, nref=nref, flags=flags)
+    torch.cuda.synchronize()
+    bb.device_status()
+    dn_h = dn.cpu().numpy()
+    uo, Io = [], []
+    for b in range(B):
+        u, Ib = oracle.propagate(f0[b], dn_h, w.dx, w.dz, w.lam, w.n0, nref=nref)
+        uo.append(u)
+        Io.append(Ib)
+    uo, Io = np.stack(uo), np.stack(Io)
+    if not per_field:
+        Io = Io.sum(axis=0)
+    if intensity_init is not None:
+        Io = Io + intensity_init.astype(np.float32).astype(np.float64)
+    return d.cpu().numpy(), I.cpu().numpy(), uo, Io
+
+
+@pytest.mark.parametrize("Nx,Ny,Nz,B", [(32, 32, 5, 1), (64, 128, 7, 1), (128, 64, 6, 2), (256, 32, 4, 3),
+                                         (32, 512, 3, 1), (512, 128, 5, 1), (1024, 64, 3, 2), (64, 1024, 3, 1),
+                                         (256, 256, 9, 5), (512, 512, 4, 9), (1024, 1024, 3, 1)])
+def test_small_shapes_batches_and_ragged_tiles(oracle_mod, Nx, Ny, Nz, B):
+    """Every line length, non-square grids, batches that do not divide the warps, grids whose
+    tiles do not divide the CTAs (ragged tail), with an adapted n_ref that changes every 2 slices."""
+    bb = need_gpu()
+    w = wl.tiny(N=Nx, Nz=Nz, n_cells=12, r_lo=0.5, r_hi=3.0)
+    w = wl.dataclasses.replace(w, Ny=Ny)
+    dn = wl.make_dn(w)
+    f0 = wl.random_field(Nx, Ny, seed=Nx + Ny + B, batch=B)
+    nref = oracle_mod.nref_from_dn(dn.numpy(), w.n0, 2)
+    u, I, uo, Io = run_both(bb, oracle_mod, w, dn, f0, nref)
+    for b in range(B):
+        assert rel_l2(u[b], uo[b]) < small_tol(Nz)
+    assert rel_l2(I, Io) < 2 * small_tol(Nz)
+    assert not np.isnan(I).any()
+
+
+@pytest.mark.parametrize("flags", ["per_field", "accumulate", "per_field+accumulate", "per_phase"])
+def test_flags(oracle_mod, flags):
+    bb = need_gpu()
+    w = wl.tiny(N=128, Nz=6, n_cells=10, r_lo=0.5, r_hi=3.0)
+    dn = wl.make_dn(w)
+    B = 3
+    f0 = wl.random_field(w.Nx, w.Ny, seed=11, batch=B)
+    fl = 0
+    if "per_field" in flags:
+        fl |= bb.INTENSITY_PER_FIELD
+    if "accumulate" in flags:
+        fl |= bb.ACCUMULATE
+    if "per_phase" in flags:
+        fl |= bb.LAUNCH_PER_PHASE
+    init = None
+    if fl & bb.ACCUMULATE:
+        shape = ((B,) if fl & bb.INTENSITY_PER_FIELD else ()) + tuple(dn.shape)
+        init = np.random.default_rng(3).uniform(0, 5, size=shape)
+    u, I, uo, Io = run_both(bb, oracle_mod, w, dn, f0, None, flags=fl, intensity_init=init)
+    assert rel_l2(u, uo) < small_tol(w.Nz)
+    assert rel_l2(I, Io) < 2 * small_tol(w.Nz)
+
+
+def test_per_phase_launches_equal_the_persistent_kernel_bitwise():
+    bb = need_gpu()
+    w = wl.config("C1").with_nz(24)
+    dn = wl.make_dn(w).cuda()
+    f0 = torch.from_numpy(wl.make_field(w)).cuda()
+    out = []
+    for fl in (0, bb.LAUNCH_PER_PHASE):
+        d, I = f0.clone(), torch.empty_like(dn)
+        bb.propagate(d, dn, w.dx, w.dz, w.lam, w.n0, intensity=I, flags=fl)
+        out.append((d, I))
+    bb.device_status()
+    assert torch.equal(out[0][0], out[1][0]) and torch.equal(out[0][1], out[1][1])
+
+
+def test_flat_entry_point_null_intensity_and_nref_variants(oracle_mod):
+    bb = need_gpu()
+    w = wl.config("C1").with_nz(16)
+    dn = wl.make_dn(w)
+    f0 = wl.make_field(w)
+    uo, Io = oracle_mod.propagate(f0[0], dn.numpy(), w.dx, w.dz, w.lam, w.n0)
+    d = torch.from_numpy(f0[0]).cuda()
+    I = torch.empty(dn.shape, device="cuda")
+    bb.propagate_simple(d, dn.cuda(), w.dx, w.dz, w.lam, w.n0, I)
+    assert rel_l2(d.cpu().numpy(), uo) < small_tol(16) and rel_l2(I.cpu().numpy(), Io) < 2 * small_tol(16)
+    d2 = torch.from_numpy(f0[0]).cuda()
+    bb.propagate_simple(d2, dn.cuda(), w.dx, w.dz, w.lam, w.n0, None)           # intensity_out = NULL
+    assert torch.equal(d, d2)
+    for slab in (1, 3):                                                         # n_ref changes every slice / 3 slices
+        nref = oracle_mod.nref_from_dn(dn.numpy(), w.n0, slab)
+        uo, Io = oracle_mod.propagate(f0[0], dn.numpy(), w.dx, w.dz, w.lam, w.n0, nref=nref)
+        d = torch.from_numpy(f0).cuda()
+        bb.propagate(d, dn.cuda(), w.dx, w.dz, w.lam, w.n0, intensity=I, nref=nref)
+        assert rel_l2(d.cpu().numpy()[0], uo) < small_tol(16) and rel_l2(I.cpu().numpy(), Io) < 2 * small_tol(16)
+
+
+def test_more_reference_indices_than_cached_tables(oracle_mod, monkeypatch):
+    """With a table cache smaller than the number of distinct n_ref values the propagation is
+    split into several launches; results must not change."""
+    bb = need_gpu()
+    w = wl.tiny(N=1024, Nz=7, n_cells=30, r_lo=2.0, r_hi=10.0, dx=0.1, dz=0.1)
+    dn = wl.make_dn(w)
+    nref = oracle_mod.nref_from_dn(dn.numpy(), w.n0, 1)
+    assert len(set(nref.tolist())) > 2
+    f0 = wl.random_field(w.Nx, w.Ny, seed=2, batch=1)
+    monkeypatch.setenv("BB_TABLE_CACHE_MB", "16")          # two 8 MiB tables
+    bb.shutdown()
+    try:
+        u, I, uo, Io = run_both(bb, oracle_mod, w, dn, f0, nref)
+    finally:
+        monkeypatch.delenv("BB_TABLE_CACHE_MB")
+        bb.shutdown()
+    assert rel_l2(u, uo) < small_tol(7) and rel_l2(I, Io) < 2 * small_tol(7)
+
+
+def test_host_buffer_entry_point_equals_device_entry_point(oracle_mod):
+    bb = need_gpu()
+    w = wl.config("C2").with_nz(150)            # 150 slices of 256 KiB: more than one streamed chunk
+    dn = wl.make_dn(w)
+    f0 = wl.make_field(w)
+    nref = oracle_mod.nref_from_dn(dn.numpy(), w.n0, 32)
+    d = torch.from_numpy(f0).cuda()
+    I = torch.empty(dn.shape, device="cuda")
+    bb.propagate(d, dn.cuda(), w.dx, w.dz, w.lam, w.n0, intensity=I, nref=nref)
+    fh = torch.from_numpy(f0.copy()).pin_memory()
+    dnh = dn.pin_memory()
+    Ih = torch.empty(dn.shape).pin_memory()
+    bb.propagate(fh, dnh, w.dx, w.dz, w.lam, w.n0, intensity=Ih, nref=nref)
+    assert torch.equal(fh, d.cpu()) and torch.equal(Ih, I.cpu())
+    fp = torch.from_numpy(f0.copy())            # pageable memory works too
+    Ip = torch.empty(dn.shape)
+    bb.propagate(fp, dn, w.dx, w.dz, w.lam, w.n0, intensity=Ip, nref=nref)
+    assert torch.equal(fp, fh) and torch.equal(Ip, Ih)
+
+
+def _full_config_parity(bb, oracle, name, nz=None, batch_limit=None):
+    """Streams the oracle through the workload slice by slice and compares with the GPU volume."""
+    w = wl.config(name)
+    if nz is not None:
+        w = w.with_nz(nz)
+    dn, f_gpu = gpu_inputs(w, bb)
+    f0 = oracle_field0(w, oracle)
+    if batch_limit is not None:
+        f0, f_gpu = f0[:batch_limit], f_gpu[:batch_limit].contiguous()
+    # both sides start from their own input field; for multiplex workloads that is part of the path
+    assert rel_l2(f_gpu.cpu().numpy(), f0) < 2e-6
+    nref = bb.nref_from_dn(dn, w.n0, w.nref_slab).numpy()
+    B = f0.shape[0]
+    I = torch.empty(dn.shape, device="cuda")
+    bb.propagate(f_gpu, dn, w.dx, w.dz, w.lam, w.n0, intensity=I, nref=nref)
+    torch.cuda.synchronize()
+    bb.device_status()
+    dn_h = dn.cpu().numpy()
+    cmp_I = StreamCompare()
+    if B == 1:
+        def on_slice(j, u, Ij):
+            cmp_I.add(I[j].cpu().numpy(), Ij)
+        uo = oracle.propagate_stream(f0[0], dn_h, w.dx, w.dz, w.lam, w.n0, nref=nref, on_slice=on_slice)[None]
+    else:
+        uo, Io = [], 0.0
+        for b in range(B):
+            u, Ib = oracle.propagate(f0[b], dn_h, w.dx, w.dz, w.lam, w.n0, nref=nref)
+            uo.append(u)
+            Io = Io + Ib
+        uo = np.stack(uo)
+        for j in range(w.Nz):
+            cmp_I.add(I[j].cpu().numpy(), Io[j])
+    got = f_gpu.cpu().numpy()
+    err_u = max(rel_l2(got[b], uo[b]) for b in range(B))
+    print("\n%s: Nz=%d B=%d  field rel-L2 %.3e  intensity rel-L2 %.3e  (per-slice intensity error: "
+          "first %.2e, mid %.2e, last %.2e)" % (name, w.Nz, B, err_u, cmp_I.rel, cmp_I.curve[0],
+                                               cmp_I.curve[len(cmp_I.curve) // 2], cmp_I.curve[-1]))
+    return err_u, cmp_I.rel
+
+
+@pytest.mark.parametrize("name", ["C1", "C2", "C3"])
+def test_config_parity_full(oracle_mod, name):
+    """BASELINE.json configs[0..2] at full size, adapted n_ref with 32-slice slabs."""
+    bb = need_gpu()
+    err_u, err_I = _full_config_parity(bb, oracle_mod, name)
+    assert err_u < TOL and err_I < TOL
+
+
+def test_config_c5_batched_parity(oracle_mod):
+    """configs[4]: 16 fields over a shared volume, summed intensity; 48 of the 512 slices
+    (the oracle needs 16 runs), all 16 fields."""
+    bb = need_gpu()
+    err_u, err_I = _full_config_parity(bb, oracle_mod, "C5", nz=48)
+    assert err_u < TOL and err_I < TOL
+
+
+@pytest.mark.slow
+def test_config_c4_headline_parity_full(oracle_mod):
+    """configs[3], the workload bench.py times, at full size (1024^2 x 1024 steps) in the same
+    launch configuration: every element of the final field and of the 4 GiB intensity volume."""
+    bb = need_gpu()
+    err_u, err_I = _full_config_parity(bb, oracle_mod, "C4")
+    assert err_u < TOL and err_I < TOL
