@@ -1,0 +1,388 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the BPM hot path on B200 (contract: see DESIGN.md "Measurement").
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: for the
+default workload C4 (BASELINE.json configs[3], the one the metric is quoted on -- ~1000
+multiplexed point sources through a 1024^3 float32 volume) that is bb_multiplex_psf
+followed by bb_propagate over all 1024 slices, i.e. ONE full propagation.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W]          # our CUDA path
+  python bench.py --impl reference ...                         # the CPU oracle, as it stands
+  torchrun --nproc-per-node N bench.py --gpus N ...            # N independent replicas
+
+Prints ONE JSON line (rank 0).  `value` is pixel-slices per second (Mvox/s) with all inputs
+resident in HBM; `e2e` is the same metric through the host-buffer entry point with the
+host<->device copies inside the timed region.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1706_02261_b200 import replicas, workloads as wl  # noqa: E402
+
+# nominal FP32 rate of the non-tensor pipe: 148 SMs x 128 lanes x 2 flop x 1.965 GHz
+# (/opt/skills/guides/B200_PROFILING.md: 148 SMs, clocks.max.sm 1965 MHz)
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+HBM_FALLBACK_GBS = 6650.0
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    except Exception:
+        return HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md)"
+
+
+def committed_dram_traffic(workload: str):
+    """DRAM bytes per launch of the persistent kernel from the committed ncu capture, or None."""
+    p = os.path.join(ROOT, "profiles", "dram_traffic.json")
+    try:
+        with open(p) as f:
+            return json.load(f).get(workload, {}).get("dram_bytes_per_launch")
+    except Exception:
+        return None
+
+
+def algorithmic_per_step(w: wl.Workload, per_field_intensity=False):
+    """Algorithmic HBM bytes, L2 bytes and flops of ONE z-step."""
+    npx = w.Nx * w.Ny
+    B = w.batch
+    hbm = 4 * npx + 4 * npx * (B if per_field_intensity else 1)
+    l2 = 32 * npx * B + 8 * npx + hbm
+    flops = (10 * npx * (math.log2(w.Nx) + math.log2(w.Ny)) + 40 * npx) * B
+    return hbm, l2, flops
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled while the timed region runs."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+              "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device_index: int):
+        self.proc = None
+        try:
+            uuid = str(torch.cuda.get_device_properties(device_index).uuid)
+            if not uuid.startswith("GPU-"):
+                uuid = "GPU-" + uuid
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", uuid, "--query-gpu=" + self.FIELDS, "--format=csv,noheader,nounits", "-lms", "50"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.06)
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except Exception:
+            self.proc.kill()
+            out = ""
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in out.strip().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 8:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1])); pw.append(float(parts[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def make_inputs(w: wl.Workload, device):
+    dn = wl.make_dn(w, device=device)
+    f0 = wl.make_field(w)
+    em = None
+    if f0 is None:
+        pos, ph, amp = wl.make_emitters(w)
+        em = tuple(torch.from_numpy(a) for a in (pos, ph, amp))
+    return dn, f0, em
+
+
+# --------------------------------------------------------------------------------------------
+def run_ours(args):
+    from paper_1706_02261_b200 import binding as bb, build
+    rank, local_rank, _ = replicas.env_world()
+    world = replicas.init()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
+    dev = torch.device("cuda", local_rank if world > 1 else 0)
+    torch.cuda.set_device(dev)
+    build.build_library()
+    bb.load()
+
+    w = wl.config(args.workload)
+    if args.nz:
+        w = w.with_nz(args.nz)
+    B, npx = w.batch, w.Nx * w.Ny
+    flags = bb.LAUNCH_PER_PHASE if args.per_phase else 0
+    dn, f0, em = make_inputs(w, dev)
+    nref = bb.nref_from_dn(dn, w.n0, w.nref_slab).numpy()
+    if em is not None:
+        em_d = tuple(t.to(dev) for t in em)
+        field = torch.empty((1, w.Ny, w.Nx), dtype=torch.complex64, device=dev)
+    else:
+        f0_d = torch.from_numpy(f0).to(dev)
+        field = torch.empty_like(f0_d)
+    inten = torch.empty((w.Nz, w.Ny, w.Nx), dtype=torch.float32, device=dev)
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def step(marks=None):
+        if em is not None:
+            bb.multiplex_psf(em_d[0], em_d[1], em_d[2], w.NA, w.Nx, w.Ny, w.dx, w.lam, out=field[0])
+        else:
+            field.copy_(f0_d)
+        if marks is not None:
+            a = ev(); a.record()
+        bb.propagate(field, dn, w.dx, w.dz, w.lam, w.n0, intensity=inten, nref=nref, flags=flags)
+        if marks is not None:
+            b = ev(); b.record()
+            marks.append((a, b))
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    bb.device_status()
+    replicas.barrier()
+    sampler = ClockSampler(dev.index) if rank == 0 else None
+    launches0 = bb.launch_count()
+    marks = []
+    e0, e1 = ev(), ev()
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(args.steps):
+        step(marks)
+    e1.record()
+    torch.cuda.synchronize()
+    replicas.barrier()
+    clocks = sampler.stop() if sampler else None
+    launches = bb.launch_count() - launches0
+    bb.device_status()
+    t_local = e0.elapsed_time(e1) * 1e-3
+    t = replicas.max_over_ranks(t_local)
+    units = float(npx) * w.Nz * B * args.steps                 # pixel-slices this rank processed
+    value = replicas.sum_over_ranks(units) / t / 1e6
+    prop_ms = statistics.mean(a.elapsed_time(b) for a, b in marks)   # the propagate call = the BPM kernel(s)
+
+    result = {
+        "metric": "pixel-slices per second through the split-step BPM (ms per full propagation = ms_per_step)",
+        "value": value, "unit": "Mvox/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": t / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "%s: %dx%d grid, %d z-slices, B=%d, dx=%g dz=%g lambda=%g n0=%g, %s, n_ref slabs of %d; "
+                               "one step = %s + bb_propagate over all slices"
+                               % (w.name, w.Nx, w.Ny, w.Nz, B, w.dx, w.dz, w.lam, w.n0,
+                                  ("%dx%d emitters NA %.2g" % (w.emitters, w.emitters, w.NA)) if em is not None else w.field,
+                                  w.nref_slab, "bb_multiplex_psf" if em is not None else "field reset"),
+                   "baseline_config": "BASELINE.json configs[%d]" % w.index,
+                   "parallelism": "replicas only (%d independent propagation(s), no collective)" % world,
+                   "l2": "inputs larger than L2: %.2f GiB dn + %.2f GiB intensity streamed per step"
+                         % (dn.numel() * 4 / 2**30, inten.numel() * 4 / 2**30),
+                   "launch_mode": "per-phase kernels" if args.per_phase else "one persistent cooperative kernel per propagation",
+                   "headline": bool(args.workload == "C4" and not args.nz)},
+        "gpu_launches": int(launches),
+        "propagate_ms": prop_ms,
+    }
+    if clocks is not None:
+        result["clocks"] = clocks
+
+    # ---- roofline of the dominant kernel (bb::bpm_kernel, one launch per propagation) ----
+    hbm_b, l2_b, flop = algorithmic_per_step(w)
+    hbm_peak, hbm_src = measured_peaks()
+    dur = prop_ms * 1e-3
+    traffic = committed_dram_traffic(w.name if not args.nz else "")
+    alu_ach = flop * w.Nz / dur / 1e12
+    result["roofline"] = {"bound": "alu", "achieved": alu_ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+                          "frac": alu_ach / FP32_PEAK_TFLOPS, "traffic": traffic,
+                          "kernel": "bb::bpm_kernel", "peak_source": "nominal 148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md)",
+                          "algorithmic_flop_per_launch": flop * w.Nz}
+    hbm_ach = hbm_b * w.Nz / dur / 1e9
+    result["roofline_hbm"] = {"bound": "hbm", "achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s",
+                              "frac": hbm_ach / hbm_peak, "traffic": traffic, "peak_source": hbm_src,
+                              "algorithmic_bytes_per_launch": hbm_b * w.Nz}
+    if rank == 0 and not args.no_probe:
+        try:
+            l2_peak = bb.probe_l2_bandwidth(32 << 20, 200, 0)
+            fp32_meas = bb.probe_fp32(20000, False)
+            l2_ach = l2_b * w.Nz / dur / 1e9
+            result["roofline_l2"] = {"bound": "l2", "achieved": l2_ach, "peak": l2_peak, "unit": "GB/s",
+                                     "frac": l2_ach / l2_peak,
+                                     "peak_source": "measured now: bb_probe_l2_bandwidth, 32 MiB resident copy",
+                                     "algorithmic_bytes_per_launch": l2_b * w.Nz}
+            result["roofline"]["peak_measured_fma_loop"] = fp32_meas
+            t_roof = max(hbm_b / (hbm_peak * 1e9), l2_b / (l2_peak * 1e9))
+            result["hbm_l2_roofline_frac"] = t_roof / (dur / w.Nz)       # T_roof / T_measured per slice
+        except Exception as e:                                            # noqa: BLE001
+            result["roofline_l2"] = {"error": str(e)}
+
+    # ---- end to end through the host-buffer entry point ----
+    if not args.no_e2e:
+        fh = torch.empty((B, w.Ny, w.Nx), dtype=torch.complex64).pin_memory()
+        dnh = torch.empty(dn.shape, dtype=torch.float32).pin_memory()
+        dnh.copy_(dn)
+        Ih = torch.empty(inten.shape, dtype=torch.float32).pin_memory()
+        if em is not None:
+            em_h = tuple(t.pin_memory() for t in em)
+        else:
+            f0_h = torch.from_numpy(f0).pin_memory()
+        h2d = dnh.numel() * 4 + fh.numel() * 8 + (sum(t.numel() * 4 for t in em) if em is not None else 0)
+        d2h = Ih.numel() * 4 + fh.numel() * 8 + (fh.numel() * 8 if em is not None else 0)
+
+        def e2e_step():
+            if em is not None:
+                d = tuple(t.to(dev, non_blocking=True) for t in em_h)
+                bb.multiplex_psf(d[0], d[1], d[2], w.NA, w.Nx, w.Ny, w.dx, w.lam, out=field[0])
+                fh.copy_(field, non_blocking=True)
+                torch.cuda.synchronize()
+            else:
+                fh.copy_(f0_h)
+            bb.propagate(fh, dnh, w.dx, w.dz, w.lam, w.n0, intensity=Ih, nref=nref, flags=flags)
+
+        n_e2e = max(1, min(args.steps, args.e2e_steps))
+        e2e_step()
+        torch.cuda.synchronize()
+        replicas.barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            e2e_step()
+        torch.cuda.synchronize()
+        t_e2e = replicas.max_over_ranks(time.perf_counter() - t0)
+        replicas.barrier()
+        e2e_val = replicas.sum_over_ranks(float(npx) * w.Nz * B * n_e2e) / t_e2e / 1e6
+        same = torch.equal(Ih[-1], inten[-1].cpu())
+        result["e2e"] = {"value": e2e_val, "unit": "Mvox/s", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                         "steps": n_e2e, "ms_per_step": t_e2e / n_e2e * 1e3, "host_memory": "pinned",
+                         "api": "bb_propagate_host (dn streamed in z-chunks, intensity streamed back)",
+                         "matches_device_path": bool(same)}
+        del dnh, Ih
+
+    # ---- the oracle on this box's host cores (reported baseline, rank 0, N = 1 only) ----
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        result["cpu_baseline"] = oracle_sample(w, dn, f0, em, nref, budget_s=args.cpu_seconds)
+
+    if rank == 0:
+        print(json.dumps(result))
+    replicas.shutdown()
+
+
+def oracle_sample(w, dn, f0, em, nref, budget_s=15.0, slices=None):
+    """Times the oracle, as it stands, on the first `slices` z-slices of the workload."""
+    import oracle
+    oracle.build()
+    if f0 is None:
+        pos, ph, amp = (t.numpy() for t in em)
+        u0 = oracle.multiplex_psf(pos, ph, amp, w.NA, w.Nx, w.Ny, w.dx, w.lam).astype(np.complex64)
+    else:
+        u0 = f0[0]
+    dn0 = dn[:1].cpu().numpy()
+    oracle.propagate_stream(u0, dn0, w.dx, w.dz, w.lam, w.n0, nref=nref[:1])          # warm-up (thread pool, caches)
+    t0 = time.perf_counter()
+    oracle.propagate_stream(u0, dn0, w.dx, w.dz, w.lam, w.n0, nref=nref[:1])
+    t1 = max(time.perf_counter() - t0, 1e-4)
+    if slices is None:
+        slices = int(min(w.Nz, max(4, budget_s / t1)))
+    dns = dn[:slices].cpu().numpy()
+    t0 = time.perf_counter()
+    oracle.propagate_stream(u0, dns, w.dx, w.dz, w.lam, w.n0, nref=nref[:slices])
+    dt = time.perf_counter() - t0
+    return {"value": w.Nx * w.Ny * slices / dt / 1e6, "unit": "Mvox/s", "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": "first %d of %d z-slices of %s, one field, double precision, %.1f s" % (slices, w.Nz, w.name, dt),
+            "seconds": dt, "slices": slices}
+
+
+# --------------------------------------------------------------------------------------------
+def run_reference(args):
+    """The reference arm for this tier is the oracle (there is no reference code): rank 0 only."""
+    rank, _, world = replicas.env_world()
+    if rank != 0:
+        return
+    import oracle
+    oracle.build()
+    w = wl.config(args.workload)
+    if args.nz:
+        w = w.with_nz(args.nz)
+    # bounded sample: S slices per step such that warmup + steps stay within ~2 minutes
+    total_steps = args.steps + args.warmup
+    probe = w.with_nz(2)
+    dn_p, f0, em = make_inputs(probe, "cpu")
+    nref_p = oracle.nref_from_dn(dn_p.numpy(), w.n0, w.nref_slab)
+    r = oracle_sample(probe, dn_p, f0, em, nref_p, slices=2)
+    per_slice = r["seconds"] / 2
+    S = int(min(w.Nz, max(2, (100.0 / total_steps) / per_slice)))
+    ws = w.with_nz(S)
+    dn, f0, em = make_inputs(ws, "cpu")
+    nref = oracle.nref_from_dn(dn.numpy(), w.n0, w.nref_slab)
+    times = []
+    for i in range(total_steps):
+        r = oracle_sample(ws, dn, f0, em, nref, slices=S)
+        if i >= args.warmup:
+            times.append(r["seconds"])
+    dt = sum(times)
+    value = w.Nx * w.Ny * S * len(times) / dt / 1e6
+    sample = "each step = first %d of %d z-slices of %s (bounded sample), one field" % (S, w.Nz, w.name)
+    print(json.dumps({
+        "impl": "reference",
+        "metric": "pixel-slices per second through the split-step BPM (ms per full propagation = ms_per_step)",
+        "value": value, "unit": "Mvox/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": dt / len(times) * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "%s (oracle, CPU): %s" % (w.name, sample), "baseline_config": "BASELINE.json configs[%d]" % w.index},
+        "cpu_baseline": {"value": value, "unit": "Mvox/s", "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "Mvox/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
+    ap.add_argument("--workload", default="C4", choices=sorted(wl.CONFIGS))
+    ap.add_argument("--nz", type=int, default=0, help="use only the first NZ slices (profiling; not the headline number)")
+    ap.add_argument("--per-phase", action="store_true", help="one kernel launch per half-step (diagnostic)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-probe", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours" and not args.nz:
+        args.warmup = 3                                   # timing rule: at least 3 warm-up steps
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -144,6 +144,17 @@ unsigned long long bb_launch_count(void); /* kernels launched by this library si
 int bb_device_status(void);             /* synchronises the device; BB_ERR_INTERNAL if a device-side
                                            watchdog tripped since the last call, else BB_OK */
 
+
+/*
+ * Measurement support: the roofline denominators MEASURED_PEAKS.json does
+ * not hold.  Synchronous; allocate and free their own buffers; not used by the BPM path.
+ * bb_probe_l2_bandwidth: GB/s over a `bytes`-sized buffer that stays in L2 (mode 0: copy, counts
+ * bytes read + written; mode 1: read only).  bb_probe_fp32: TFLOP/s of dependent-free FMA chains,
+ * packed = 0 scalar FFMA, 1 = FFMA2 (fma.rn.f32x2).
+ */
+int bb_probe_l2_bandwidth(unsigned long long bytes, int iters, int mode, double *gb_per_s);
+int bb_probe_fp32(int iters, int packed, double *tflops);
+
 #ifdef __cplusplus
 }
 #endif

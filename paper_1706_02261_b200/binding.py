@@ -21,7 +21,7 @@ LAUNCH_PER_PHASE = 4
 
 EXPORTS = ("bb_propagate", "bb_propagate_ex", "bb_propagate_host", "bb_nref_from_dn",
            "bb_multiplex_psf", "bb_fft2", "bb_propagator_table", "bb_last_error", "bb_version",
-           "bb_shutdown", "bb_launch_count", "bb_device_status")
+           "bb_shutdown", "bb_launch_count", "bb_device_status", "bb_probe_l2_bandwidth", "bb_probe_fp32")
 
 STATUS_NAMES = {0: "BB_OK", 1: "BB_ERR_INVALID_ARG", 2: "BB_ERR_UNSUPPORTED_SHAPE", 3: "BB_ERR_CUDA",
                 4: "BB_ERR_OOM", 5: "BB_ERR_ARCH", 6: "BB_ERR_INTERNAL"}
@@ -60,6 +60,8 @@ def load() -> ctypes.CDLL:
     lib.bb_multiplex_psf.argtypes = [vp, vp, vp, i, f, i, i, f, f, vp, vp]
     lib.bb_fft2.argtypes = [vp, i, i, i, i, vp]
     lib.bb_propagator_table.argtypes = [i, i, f, f, f, f, vp, vp]
+    lib.bb_probe_l2_bandwidth.argtypes = [ctypes.c_ulonglong, i, i, ctypes.POINTER(ctypes.c_double)]
+    lib.bb_probe_fp32.argtypes = [i, i, ctypes.POINTER(ctypes.c_double)]
     lib.bb_last_error.restype = ctypes.c_char_p
     lib.bb_launch_count.restype = ctypes.c_ulonglong
     lib.bb_shutdown.restype = None
@@ -191,6 +193,20 @@ def propagator_table(Nx: int, Ny: int, dx: float, dz: float, lam: float, nref: f
     with torch.cuda.device(out.device):
         _check(lib.bb_propagator_table(Nx, Ny, dx, dz, lam, nref, ctypes.c_void_p(out.data_ptr()), _stream_ptr(stream)))
     return out
+
+
+def probe_l2_bandwidth(nbytes: int = 32 << 20, iters: int = 200, mode: int = 0) -> float:
+    """GB/s of an L2-resident copy (mode 0) or read (mode 1); see ``bb_probe_l2_bandwidth``."""
+    out = ctypes.c_double()
+    _check(load().bb_probe_l2_bandwidth(nbytes, iters, mode, ctypes.byref(out)))
+    return out.value
+
+
+def probe_fp32(iters: int = 20000, packed: bool = False) -> float:
+    """TFLOP/s of the scalar or packed FP32 FMA pipe; see ``bb_probe_fp32``."""
+    out = ctypes.c_double()
+    _check(load().bb_probe_fp32(iters, 1 if packed else 0, ctypes.byref(out)))
+    return out.value
 
 
 def device_status():
