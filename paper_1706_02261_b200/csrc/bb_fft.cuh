@@ -148,23 +148,48 @@ template <int T, int CW> struct ColGeom {
     static constexpr int TILE = T == 1 ? 0 : CW * RS;                 // float2 per tile slot
 };
 
-struct SyncWarp  { __device__ __forceinline__ void operator()() const { __syncwarp(); } };
-struct SyncBlock { __device__ __forceinline__ void operator()() const { __syncthreads(); } };
+// Team synchronisation of the transposes: a row line lives in one warp, a column tile spans the CTA.
+struct SyncSel {
+    bool warp;
+    __device__ __forceinline__ void operator()() const {
+        if (warp) __syncwarp();
+        else __syncthreads();
+    }
+};
 
-// One line FFT (see file header).  v: this thread's 32 points x[t + T*j].
-//   tw   : shared, [32][T], tw[k1*T + t] = exp(-2 pi i k1 t / N)  (conjugated for SIGN = +1)
+// One forward line FFT (see file header).  v: this thread's 32 points x[t + T*j].
+//   tw   : shared, [32][T], tw[k1*T + t] = exp(-2 pi i k1 t / N)
 //   ybuf : shared, base of this thread's line region; S = stride between k1 rows
-template <int T, int SIGN, int S, class Sync>
-__device__ __forceinline__ void line_fft(cf (&v)[32], const cf *__restrict__ tw, cf *ybuf, int t, Sync sync) {
-    Dft<32, SIGN>::run(v);
-    if constexpr (T > 1) {
+// The inverse transform is conj . forward . conj (done by the caller), so that one copy of this
+// code serves both directions.  For T = 32 the two radix-32 stages are a rolled loop over the
+// same butterfly code.
+template <int T, int S, class Sync>
+__device__ __forceinline__ void line_fft_fwd(cf (&v)[32], const cf *__restrict__ tw, cf *ybuf, int t, Sync sync) {
+    if constexpr (T == 1) {
+        Dft<32, -1>::run(v);
+    } else if constexpr (T == 32) {
+#pragma unroll 1
+        for (int stage = 0; stage < 2; ++stage) {
+            Dft<32, -1>::run(v);
+            if (stage == 0) {
+#pragma unroll
+                for (int k1 = 0; k1 < 32; ++k1) {
+                    cf x = v[k1];
+                    if (k1 > 0) x = cmul(x, tw[k1 * T + t]);
+                    ybuf[k1 * S + t] = x;
+                }
+                sync();
+#pragma unroll
+                for (int n2 = 0; n2 < 32; ++n2) v[n2] = ybuf[t * S + n2];
+                sync();
+            }
+        }
+    } else {
+        Dft<32, -1>::run(v);
 #pragma unroll
         for (int k1 = 0; k1 < 32; ++k1) {
             cf x = v[k1];
-            if (k1 > 0) {
-                cf w = tw[k1 * T + t];
-                x = SIGN < 0 ? cmul(x, w) : cmulc(x, w);
-            }
+            if (k1 > 0) x = cmul(x, tw[k1 * T + t]);
             ybuf[k1 * S + t] = x;
         }
         sync();
@@ -174,7 +199,7 @@ __device__ __forceinline__ void line_fft(cf (&v)[32], const cf *__restrict__ tw,
             cf w[T];
 #pragma unroll
             for (int n2 = 0; n2 < T; ++n2) w[n2] = ybuf[(t + T * m) * S + n2];
-            Dft<T, SIGN>::run(w);
+            Dft<T, -1>::run(w);
 #pragma unroll
             for (int k2 = 0; k2 < T; ++k2) v[m + G * k2] = w[k2];
         }
