@@ -17,6 +17,7 @@ OBJ = os.path.join(HERE, "_build")
 LIB = os.path.join(HERE, "libbiobeam_b200.so")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 TXS = (1, 2, 4, 8, 16, 32)
+PXS = (1, 2, 4)
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I", INCLUDE]
@@ -56,6 +57,9 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
     for tx in TXS:
         obj = os.path.join(OBJ, "bb_inst_tx%d.o" % tx)
         jobs.append((obj, [nvcc, *NVCC_FLAGS, "-DBB_TX=%d" % tx, "-c", os.path.join(CSRC, "bb_inst.cu"), "-o", obj]))
+    for px in PXS:
+        obj = os.path.join(OBJ, "bb_inst16_px%d.o" % px)
+        jobs.append((obj, [nvcc, *NVCC_FLAGS, "-DBB_PX=%d" % px, "-c", os.path.join(CSRC, "bb_inst16.cu"), "-o", obj]))
     obj_api = os.path.join(OBJ, "bb_api.o")
     jobs.append((obj_api, [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, "bb_api.cu"), "-o", obj_api]))
     obj_probe = os.path.join(OBJ, "bb_probe.o")

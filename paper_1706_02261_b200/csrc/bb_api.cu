@@ -56,6 +56,7 @@ int log2_exact(int n) {
 // ------------------------------------------------------------------------------------------
 struct TableKey {
     float dx, dz, lambda, nref;
+    int perm;                      // column order: 1 natural, P = kx-class-major (16-point-thread kernel)
     bool operator==(const TableKey &o) const {
         return memcmp(this, &o, sizeof(TableKey)) == 0;
     }
@@ -65,6 +66,8 @@ struct TableEntry { TableKey key; cf *ptr; unsigned long long last_use; };
 struct Plan {
     int device, Nx, Ny;
     cf *twx = nullptr, *twy = nullptr;
+    cf *tw256 = nullptr, *twcx = nullptr, *twcy = nullptr;   // 16-point-thread kernel tables
+    bool k16 = false;              // that kernel is available for this shape
     unsigned *bar = nullptr;
     int *status = nullptr;
     std::vector<TableEntry> tables;
@@ -131,6 +134,36 @@ int get_plan(int Nx, int Ny, Plan **out) {
     BB_CUDA(cudaMalloc(&p->status, 256));
     BB_CUDA(cudaMemset(p->bar, 0, 256));
     BB_CUDA(cudaMemset(p->status, 0, 256));
+    if (bb::kernel16_supports(Nx, Ny) && !getenv("BB_DISABLE_K16")) {
+        // sub-line twiddles exp(-2 pi i k1 t / 256) and class twiddles exp(-2 pi i c q / N), c = 1..P-1, q < 256
+        std::vector<cf> t256(256);
+        for (int k1 = 0; k1 < 16; ++k1)
+            for (int t = 0; t < 16; ++t) {
+                double ph = -kTwoPi * (double)(k1 * t) / 256.0;
+                t256[(size_t)k1 * 16 + t] = make_float2((float)cos(ph), (float)sin(ph));
+            }
+        auto class_tw = [](int N) {
+            int P = N / 256;
+            std::vector<cf> w((size_t)std::max(1, (P - 1) * 256));
+            for (int c = 1; c < P; ++c)
+                for (int q = 0; q < 256; ++q) {
+                    double ph = -kTwoPi * (double)(c * q) / (double)N;
+                    w[(size_t)(c - 1) * 256 + q] = make_float2((float)cos(ph), (float)sin(ph));
+                }
+            return w;
+        };
+        std::vector<cf> cx = class_tw(Nx), cy = class_tw(Ny);
+        BB_CUDA(cudaMalloc(&p->tw256, t256.size() * sizeof(cf)));
+        BB_CUDA(cudaMalloc(&p->twcx, cx.size() * sizeof(cf)));
+        BB_CUDA(cudaMalloc(&p->twcy, cy.size() * sizeof(cf)));
+        BB_CUDA(cudaMemcpy(p->tw256, t256.data(), t256.size() * sizeof(cf), cudaMemcpyHostToDevice));
+        BB_CUDA(cudaMemcpy(p->twcx, cx.data(), cx.size() * sizeof(cf), cudaMemcpyHostToDevice));
+        BB_CUDA(cudaMemcpy(p->twcy, cy.data(), cy.size() * sizeof(cf), cudaMemcpyHostToDevice));
+        int rc16 = bb::kernel16_prepare(Nx, Ny);
+        if (rc16 != 0) { delete p; return fail(BB_ERR_CUDA, "kernel16_prepare failed: %s", cudaGetErrorString((cudaError_t)rc16)); }
+        if (bb::kernel16_blocks_per_sm(Nx, Ny) < 1) { delete p; return fail(BB_ERR_CUDA, "16-point BPM kernel does not fit on an SM"); }
+        p->k16 = true;
+    }
     size_t tb = (size_t)Nx * Ny * sizeof(cf);
     p->table_capacity = std::max<size_t>(2, std::min<size_t>(4096, table_budget_bytes() / tb));
     rc = bb::kernel_prepare(Nx, Ny);
@@ -158,7 +191,7 @@ int build_table(Plan *p, const TableKey &k, cf *dst, cudaStream_t s) {
     double kk = k0 * (double)k.nref;
     dim3 block(128), grid((p->Nx + 127) / 128, p->Ny);
     bb::propagator_table_kernel<<<grid, block, 0, s>>>(dst, p->Nx, p->Ny, (double)k.dx, (double)k.dz, kk,
-                                                       1.0 / ((double)p->Nx * (double)p->Ny));
+                                                       1.0 / ((double)p->Nx * (double)p->Ny), k.perm);
     ++g_launches;
     BB_CUDA(cudaGetLastError());
     return BB_OK;
@@ -221,6 +254,10 @@ int validate_common(const void *field, const float *dn, int Nx, int Ny, int Nz, 
     return BB_OK;
 }
 
+// The 16-point-thread kernel serves single fields on 256/512/1024 grids; everything else (batches,
+// other shapes, the generic transform programs) runs on the 32-point-thread kernel.
+bool use_k16(const Plan *p, int B) { return p->k16 && B == 1; }
+
 int batch_warps(int B) {
     int bw = 1;
     while (bw < B && bw < bb::kWarps) bw <<= 1;
@@ -239,19 +276,25 @@ int launch_steps(Plan *p, cf *field, const float *dn, float *inten, long long in
     P.Nz_total = Nz_total; P.j_base = j0;
     P.mode = 0;
     P.twx = p->twx; P.twy = p->twy; P.bar = p->bar; P.status = p->status;
+    P.tw256 = p->tw256; P.twcx = p->twcx; P.twcy = p->twcy;
     P.flags = flags & 3u;
+    const bool k16 = use_k16(p, B);
+    auto launch = [&](bool coop) {
+        return k16 ? bb::kernel16_launch(p->Nx, p->Ny, P, p->grid, coop, s)
+                   : bb::kernel_launch(p->Nx, p->Ny, P, p->grid, coop, s);
+    };
     int p0 = (j0 == 0) ? 0 : 2 * j0 + 1, p1 = 2 * j1 + 1;
     if (flags & BB_LAUNCH_PER_PHASE) {
         for (int ph = p0; ph < p1; ++ph) {
             P.p0 = ph; P.p1 = ph + 1;
-            cudaError_t e = bb::kernel_launch(p->Nx, p->Ny, P, p->grid, false, s);
+            cudaError_t e = launch(false);
             ++g_launches;
             if (e != cudaSuccess) return fail(BB_ERR_CUDA, "phase launch failed: %s", cudaGetErrorString(e));
         }
     } else {
         P.p0 = p0; P.p1 = p1;
         BB_CUDA(cudaMemsetAsync(p->bar, 0, sizeof(unsigned), s));
-        cudaError_t e = bb::kernel_launch(p->Nx, p->Ny, P, p->grid, true, s);
+        cudaError_t e = launch(true);
         ++g_launches;
         if (e != cudaSuccess) return fail(BB_ERR_CUDA, "cooperative launch failed: %s", cudaGetErrorString(e));
     }
@@ -260,7 +303,7 @@ int launch_steps(Plan *p, cf *field, const float *dn, float *inten, long long in
 
 // Per-step tables and phase offsets for steps [j0, *j_done): the longest prefix of [j0, Nz)
 // whose distinct propagator tables fit the cache together (normally all of it).
-int prepare_steps(Plan *p, int Nz, int j0, float dx, float dz, float lambda, float n0, const float *nref,
+int prepare_steps(Plan *p, int B, int Nz, int j0, float dx, float dz, float lambda, float n0, const float *nref,
                   cudaStream_t s, std::vector<const cf *> &h_tab, std::vector<float> &h_phase, int *j_done) {
     double k0 = kTwoPi / (double)lambda;
     unsigned long long protect = ++p->tick;
@@ -270,7 +313,7 @@ int prepare_steps(Plan *p, int Nz, int j0, float dx, float dz, float lambda, flo
     for (; j < Nz; ++j) {
         float nr = nref ? nref[j] : n0;
         if (!(last_ptr && nr == last_nref)) {
-            TableKey key = {dx, dz, lambda, nr};
+            TableKey key = {dx, dz, lambda, nr, use_k16(p, B) ? p->Nx / 256 : 1};
             cf *ptr = nullptr;
             int rc = get_table(p, key, s, protect, &ptr);
             if (rc == kTableCacheFull) break;                 // the rest goes into the next launch
@@ -338,6 +381,28 @@ cudaError_t kernel_launch(int Nx, int Ny, const KParams &P, int grid, bool coop,
     BB_SWITCH_TX(launch, Ny / 32, P, grid, coop, s)
     return cudaErrorInvalidValue;
 }
+#define BB_SWITCH_PX(fn, ...)                           \
+    switch (Nx / 256) {                                 \
+        case 1: return inst16_1_##fn(__VA_ARGS__);      \
+        case 2: return inst16_2_##fn(__VA_ARGS__);      \
+        case 4: return inst16_4_##fn(__VA_ARGS__);      \
+    }
+bool kernel16_supports(int Nx, int Ny) {
+    auto ok = [](int n) { return n == 256 || n == 512 || n == 1024; };
+    return ok(Nx) && ok(Ny);
+}
+int kernel16_prepare(int Nx, int Ny) {
+    BB_SWITCH_PX(prepare, Ny / 256)
+    return (int)cudaErrorInvalidValue;
+}
+int kernel16_blocks_per_sm(int Nx, int Ny) {
+    BB_SWITCH_PX(blocks_per_sm, Ny / 256)
+    return 0;
+}
+cudaError_t kernel16_launch(int Nx, int Ny, const KParams &P, int grid, bool coop, cudaStream_t s) {
+    BB_SWITCH_PX(launch, Ny / 256, P, grid, coop, s)
+    return cudaErrorInvalidValue;
+}
 }  // namespace bb
 
 // ==========================================================================================
@@ -352,6 +417,7 @@ void bb_shutdown(void) {
     cudaDeviceSynchronize();
     for (Plan *p : g_plans) {
         cudaFree(p->twx); cudaFree(p->twy); cudaFree(p->bar); cudaFree(p->status);
+        if (p->tw256) { cudaFree(p->tw256); cudaFree(p->twcx); cudaFree(p->twcy); }
         for (TableEntry &e : p->tables) cudaFree(e.ptr);
         if (p->d_htab) cudaFree((void *)p->d_htab);
         if (p->d_phase) cudaFree(p->d_phase);
@@ -398,7 +464,7 @@ int bb_propagate_ex(void *field, const float *dn, int Nx, int Ny, int Nz, float 
     int j0 = 0;
     while (j0 < Nz) {
         int j1;
-        rc = prepare_steps(p, Nz, j0, dx, dz, lambda, n0, nref, s, h_tab, h_phase, &j1);
+        rc = prepare_steps(p, B, Nz, j0, dx, dz, lambda, n0, nref, s, h_tab, h_phase, &j1);
         if (rc) return rc;
         if (j1 <= j0) return fail(BB_ERR_OOM, "propagator table cache too small for one step");
         rc = launch_steps(p, (cf *)field, dn + (size_t)j0 * npx,
@@ -485,7 +551,7 @@ int bb_propagate_host(void *field_host, const float *dn_host, int Nx, int Ny, in
         int ja = j0;
         while (ja < j1) {
             if (ja >= prepared) {
-                rc = prepare_steps(p, Nz, ja, dx, dz, lambda, n0, nref, s_run, h_tab, h_phase, &prepared);
+                rc = prepare_steps(p, B, Nz, ja, dx, dz, lambda, n0, nref, s_run, h_tab, h_phase, &prepared);
                 if (rc || prepared <= ja) { cleanup(); return rc ? rc : fail(BB_ERR_OOM, "propagator table cache too small"); }
             }
             int jb = std::min(j1, prepared);
@@ -589,7 +655,7 @@ int bb_propagator_table(int Nx, int Ny, float dx, float dz, float lambda, float 
     Plan *p;
     int rc = get_plan(Nx, Ny, &p);
     if (rc) return rc;
-    TableKey k = {dx, dz, lambda, nref};
+    TableKey k = {dx, dz, lambda, nref, 1};
     return build_table(p, k, (cf *)out, (cudaStream_t)stream);
 }
 

@@ -10,13 +10,17 @@ __device__ __forceinline__ int freq_index(int p, int n) { return (p < n / 2) ? p
 
 // H[q][p] = (s > 0) ? exp(i dz sqrt(s)) * inv_norm : 0,  s = k^2 - kx^2 - ky^2   (bb.h; reading A2).
 // Everything in double, no fused multiply-adds in s (the cut-off test is a decision).
+// perm > 1: column p holds DFT bin perm * (p mod Nx/perm) + p / (Nx/perm), the kx-class-major order in
+// which the 16-point-thread kernel keeps the field between its phases (bb_kernels16.cuh).
 __global__ void propagator_table_kernel(float2 *__restrict__ H, int Nx, int Ny, double dx, double dz,
-                                        double k, double inv_norm) {
+                                        double k, double inv_norm, int perm) {
     const double two_pi = 6.283185307179586476925286766559;
     int p = blockIdx.x * blockDim.x + threadIdx.x;
     int q = blockIdx.y;
     if (p >= Nx) return;
-    double kx = __ddiv_rn(__dmul_rn(two_pi, (double)freq_index(p, Nx)), __dmul_rn((double)Nx, dx));
+    const int Lc = Nx / perm;
+    const int bin = perm * (p % Lc) + p / Lc;
+    double kx = __ddiv_rn(__dmul_rn(two_pi, (double)freq_index(bin, Nx)), __dmul_rn((double)Nx, dx));
     double ky = __ddiv_rn(__dmul_rn(two_pi, (double)freq_index(q, Ny)), __dmul_rn((double)Ny, dx));
     double s = __dsub_rn(__dsub_rn(__dmul_rn(k, k), __dmul_rn(kx, kx)), __dmul_rn(ky, ky));
     float2 h = make_float2(0.f, 0.f);

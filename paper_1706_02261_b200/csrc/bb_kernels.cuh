@@ -47,6 +47,7 @@ struct KParams {
     int mode;                  // 0: BPM phase sequence, 1: prog[]
     PhaseProg prog[2];
     const cf *twx, *twy;       // global twiddle tables [32][T]
+    const cf *tw256, *twcx, *twcy;   // 16-point-thread kernel: sub-line twiddles [16][16], class twiddles [P-1][256]
     unsigned *bar;             // grid barrier counter (zeroed before the launch)
     int *status;               // device flag: != 0 -> watchdog tripped
     unsigned flags;            // BB_ACCUMULATE = 1, BB_INTENSITY_PER_FIELD = 2

@@ -18,9 +18,23 @@ BB_DECLARE_INST(16)
 BB_DECLARE_INST(32)
 #undef BB_DECLARE_INST
 
+// 16-point-thread kernel (bb_kernels16.cuh), one set per PX = Nx/256 in {1, 2, 4}; bb_inst16.cu.
+#define BB_DECLARE_INST16(PX)                                                                      \
+    cudaError_t inst16_##PX##_prepare(int PY);                                                     \
+    int inst16_##PX##_blocks_per_sm(int PY);                                                       \
+    cudaError_t inst16_##PX##_launch(int PY, const KParams &P, int grid, bool coop, cudaStream_t s);
+BB_DECLARE_INST16(1)
+BB_DECLARE_INST16(2)
+BB_DECLARE_INST16(4)
+#undef BB_DECLARE_INST16
+
 // Dispatch on (Nx, Ny); defined in bb_api.cu.
 int kernel_prepare(int Nx, int Ny);           // returns a cudaError_t value
 int kernel_blocks_per_sm(int Nx, int Ny);
 cudaError_t kernel_launch(int Nx, int Ny, const KParams &P, int grid, bool coop, cudaStream_t s);
+bool kernel16_supports(int Nx, int Ny);
+int kernel16_prepare(int Nx, int Ny);
+int kernel16_blocks_per_sm(int Nx, int Ny);
+cudaError_t kernel16_launch(int Nx, int Ny, const KParams &P, int grid, bool coop, cudaStream_t s);
 
 }  // namespace bb
