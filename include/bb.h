@@ -154,6 +154,14 @@ int bb_device_status(void);             /* synchronises the device; BB_ERR_INTER
  */
 int bb_probe_l2_bandwidth(unsigned long long bytes, int iters, int mode, double *gb_per_s);
 int bb_probe_fp32(int iters, int packed, double *tflops);
+/*
+ * bb_probe_trace: timeline of the persistent kernel, for profiling only.  device_buf is a DEVICE
+ * long long[phases][grid][6] (grid = SM count) or NULL to switch tracing off.  While set, every
+ * single-field propagation of at most (phases - 1) / 2 steps on a 256/512/1024 grid records, per
+ * phase and CTA, the SM clock at phase start, work done, barrier arrived, pointwise factors staged
+ * and barrier released, and the global nanosecond timer at release.
+ */
+int bb_probe_trace(long long *device_buf, int phases);
 
 #ifdef __cplusplus
 }

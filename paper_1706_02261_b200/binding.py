@@ -21,7 +21,7 @@ LAUNCH_PER_PHASE = 4
 
 EXPORTS = ("bb_propagate", "bb_propagate_ex", "bb_propagate_host", "bb_nref_from_dn",
            "bb_multiplex_psf", "bb_fft2", "bb_propagator_table", "bb_last_error", "bb_version",
-           "bb_shutdown", "bb_launch_count", "bb_device_status", "bb_probe_l2_bandwidth", "bb_probe_fp32")
+           "bb_shutdown", "bb_launch_count", "bb_device_status", "bb_probe_l2_bandwidth", "bb_probe_fp32", "bb_probe_trace")
 
 STATUS_NAMES = {0: "BB_OK", 1: "BB_ERR_INVALID_ARG", 2: "BB_ERR_UNSUPPORTED_SHAPE", 3: "BB_ERR_CUDA",
                 4: "BB_ERR_OOM", 5: "BB_ERR_ARCH", 6: "BB_ERR_INTERNAL"}
@@ -62,6 +62,7 @@ def load() -> ctypes.CDLL:
     lib.bb_propagator_table.argtypes = [i, i, f, f, f, f, vp, vp]
     lib.bb_probe_l2_bandwidth.argtypes = [ctypes.c_ulonglong, i, i, ctypes.POINTER(ctypes.c_double)]
     lib.bb_probe_fp32.argtypes = [i, i, ctypes.POINTER(ctypes.c_double)]
+    lib.bb_probe_trace.argtypes = [ctypes.c_void_p, i]
     lib.bb_last_error.restype = ctypes.c_char_p
     lib.bb_launch_count.restype = ctypes.c_ulonglong
     lib.bb_shutdown.restype = None
@@ -223,3 +224,14 @@ def version() -> int:
 
 def shutdown():
     load().bb_shutdown()
+
+
+def probe_trace(buf: Optional[torch.Tensor]) -> None:
+    """Switch the persistent kernel's timeline on (``buf``: CUDA int64 [phases][grid][6]) or off (None);
+    see ``bb_probe_trace``."""
+    if buf is None:
+        _check(load().bb_probe_trace(None, 0))
+        return
+    if not (buf.is_cuda and buf.dtype == torch.int64 and buf.is_contiguous() and buf.dim() == 3 and buf.shape[2] == 6):
+        raise ValueError("trace buffer must be a contiguous CUDA int64 tensor [phases][grid][6]")
+    _check(load().bb_probe_trace(buf.data_ptr(), int(buf.shape[0])))

@@ -23,6 +23,8 @@ typedef float2 cf;
 thread_local std::string g_err;
 std::mutex g_mu;
 unsigned long long g_launches = 0;
+long long *g_trace = nullptr;      // bb_probe_trace
+int g_trace_phases = 0;
 
 int fail(int code, const char *fmt, ...) {
     char buf[512];
@@ -279,6 +281,8 @@ int launch_steps(Plan *p, cf *field, const float *dn, float *inten, long long in
     P.tw256 = p->tw256; P.twcx = p->twcx; P.twcy = p->twcy;
     P.flags = flags & 3u;
     const bool k16 = use_k16(p, B);
+    { const char *e = getenv("BB_DBG"); P.dbg = e ? atoi(e) : 0; }
+    if (g_trace && k16 && 2 * j1 + 1 <= g_trace_phases) { P.trace = g_trace; P.trace_p0 = 0; }
     auto launch = [&](bool coop) {
         return k16 ? bb::kernel16_launch(p->Nx, p->Ny, P, p->grid, coop, s)
                    : bb::kernel_launch(p->Nx, p->Ny, P, p->grid, coop, s);
@@ -619,6 +623,13 @@ int bb_nref_from_dn(const float *dn, int Nx, int Ny, int Nz, float n0, int slab,
         float v = (float)((double)n0 + mean);
         for (int j = j0; j < j1; ++j) nref_out[j] = v;
     }
+    return BB_OK;
+}
+
+int bb_probe_trace(long long *device_buf, int phases) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    g_trace = device_buf;
+    g_trace_phases = device_buf ? phases : 0;
     return BB_OK;
 }
 

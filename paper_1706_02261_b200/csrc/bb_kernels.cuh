@@ -51,6 +51,9 @@ struct KParams {
     unsigned *bar;             // grid barrier counter (zeroed before the launch)
     int *status;               // device flag: != 0 -> watchdog tripped
     unsigned flags;            // BB_ACCUMULATE = 1, BB_INTENSITY_PER_FIELD = 2
+    long long *trace;          // bb_probe_trace: [phase - trace_p0][CTA][6] time stamps, or nullptr
+    int trace_p0;
+    int dbg;
 };
 
 __device__ __forceinline__ cf ld_cg(const cf *p) { return __ldcg(p); }

@@ -29,10 +29,11 @@ template <int PX, int PY>
 struct Smem16 {
     static constexpr int kTw = 256;                                   // sub-line twiddles [16][16]
     static constexpr int kTwc = (PX - 1) * kL + (PY - 1) * kL;          // class twiddles, x then y
-    static constexpr int kY = (kThreads16 / 16) * 16 * 17;              // sub-line transposes
-    static constexpr int kX = kThreads16 * 16;                          // class exchange
-    static constexpr int kPw = kThreads16 * 16;                         // pointwise factors
-    static constexpr size_t bytes = (size_t)(kTw + kTwc + kY + kX + kPw) * sizeof(cf) + 16;
+    static constexpr int kY = (kThreads16 / 16) * 16 * 17;              // sub-line transposes; the class exchange
+                                                                        // (kThreads16 * 16) reuses the same region
+    static constexpr int kPw = kThreads16 * 16;                         // pointwise factors: one buffer for the
+                                                                        // propagator values, one for the screen
+    static constexpr size_t bytes = (size_t)(kTw + kTwc + kY + 2 * kPw) * sizeof(cf) + 16;
 };
 
 struct Phase16 {
@@ -99,6 +100,41 @@ struct TeamSync {
     __device__ __forceinline__ void operator()() const { tm.sync(); }
 };
 
+// sin and cos of the phase-screen argument (bb.h step 4).  Arguments are k0 dz (n - n_ref), a
+// fraction of a radian for any sample a BPM step is valid for: three-term Cody-Waite reduction by
+// pi/2 and degree-7/8 polynomials on [-pi/4, pi/4] (weighted least-squares fits, max abs error
+// 4.5e-8 / 7.4e-8 in float32, i.e. half an ulp of 1), without the large-argument path of sincosf
+// that made the staging 28 % of a row phase (profiles/r01_b).  Huge arguments take the library path.
+__device__ __forceinline__ void screen_sincos(float a, float &sn, float &cs) {
+    if (fabsf(a) > 4096.f) { sincosf(a, &sn, &cs); return; }
+    const float k = rintf(a * 6.366197467e-01f);
+    float r = fmaf(k, -1.570796371e+00f, a);
+    r = fmaf(k, 4.371138829e-08f, r);
+    r = fmaf(k, 1.776356839e-15f, r);
+    const int q = (int)k;
+    const float r2 = r * r;
+    float sp = fmaf(-1.9513932562e-04f, r2, 8.3321482563e-03f);
+    sp = fmaf(sp, r2, -1.6666654339e-01f);
+    const float s0 = fmaf(r * r2, sp, r);
+    float cp = fmaf(2.4435851735e-05f, r2, -1.3887341487e-03f);
+    cp = fmaf(cp, r2, 4.1666646237e-02f);
+    const float c0 = fmaf(r2 * r2, cp, fmaf(-0.5f, r2, 1.f));
+    const float s1 = (q & 1) ? c0 : s0, c1 = (q & 1) ? s0 : c0;
+    sn = (q & 2) ? -s1 : s1;
+    cs = ((q + 1) & 2) ? -c1 : c1;
+}
+
+// The same for arguments already known to lie in [-pi/4, pi/4] (the usual case: |k0 dz dn| << 1).
+__device__ __forceinline__ void screen_sincos_small(float r, float &sn, float &cs) {
+    const float r2 = r * r;
+    float sp = fmaf(-1.9513932562e-04f, r2, 8.3321482563e-03f);
+    sp = fmaf(sp, r2, -1.6666654339e-01f);
+    sn = fmaf(r * r2, sp, r);
+    float cp = fmaf(2.4435851735e-05f, r2, -1.3887341487e-03f);
+    cp = fmaf(cp, r2, 4.1666646237e-02f);
+    cs = fmaf(r2 * r2, cp, fmaf(-0.5f, r2, 1.f));
+}
+
 // Pointwise factors of the unit the thread works on, slot (jp, m) -> pw[(jp*P + m) * kThreads16]:
 // kind 1: exp(i (pb dn + pa)) at pixel n = q(jp) + 256 m of row `unit` of a dn slice (bb.h step 4);
 // kind 2: table value H[n][column] of column tile `unit` (bb.h step 2).  Runs off the critical
@@ -114,11 +150,26 @@ __device__ __forceinline__ void fill_pw16(int kind, const void *src, int unit, f
         for (int jp = 0; jp < JP; ++jp)
 #pragma unroll
             for (int m = 0; m < P; ++m) x[jp * P + m] = __ldcs(dnp + tm.q(jp) + kL * m);
-#pragma unroll 4
+        float amax = 0.f;
+#pragma unroll
         for (int i = 0; i < 16; ++i) {
-            float s, c;
-            sincosf(fmaf(pb, x[i], pa), &s, &c);
-            pw[i * kThreads16] = make_float2(c, s);
+            x[i] = fmaf(pb, x[i], pa);
+            amax = fmaxf(amax, fabsf(x[i]));
+        }
+        if (__all_sync(__activemask(), amax <= 0.78539816f)) {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+                float s, c;
+                screen_sincos_small(x[i], s, c);
+                pw[i * kThreads16] = make_float2(c, s);
+            }
+        } else {
+#pragma unroll 2
+            for (int i = 0; i < 16; ++i) {
+                float s, c;
+                screen_sincos(x[i], s, c);
+                pw[i * kThreads16] = make_float2(c, s);
+            }
         }
     } else {
         const cf *hp = reinterpret_cast<const cf *>(src) + (long long)unit * CW + tm.col;
@@ -136,7 +187,7 @@ __device__ __forceinline__ void fill_pw16(int kind, const void *src, int unit, f
 // ----------------------------------------------------------------------------------------
 template <int P, int CW, bool ROW, int NX, int NY>
 __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, const cf *sm_tw, const cf *sm_twc,
-                                            cf *sm_y, cf *sm_x, cf *sm_pw, PwTag &tag) {
+                                            cf *sm_y, cf *sm_pw, PwTag &tag) {
     typedef Team16<P, CW> TM;
     constexpr int S1 = ROW ? +1 : -1, S2 = -S1;
     constexpr int JP = TM::JP;
@@ -148,7 +199,7 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
     const int a0 = (int)(((long long)NU * blockIdx.x) / gridDim.x);
     const int a1 = (int)(((long long)NU * (blockIdx.x + 1)) / gridDim.x);
     cf *ybuf = sm_y + ((threadIdx.x / (16 * CW)) * (16 * 17 * CW)) + tm.col;        // one region per (team, class)
-    cf *xbuf = sm_x + tm.team * (TM::TEAM * 16) + tm.col;
+    cf *xbuf = sm_y + tm.team * (TM::TEAM * 17) + tm.col;                            // same memory, team's part
     cf *pw = sm_pw + threadIdx.x;
     const bool want_I = d.kind == 1 && K.inten != nullptr;
     const bool accumulate = (K.flags & 1u) != 0;
@@ -171,6 +222,7 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
             else subline_fft<S1, CW>(v, sm_tw, ybuf, tm.t, tsync);
             if constexpr (P > 1) {
                 // exchange: (class, 16 indices) -> (group, 16/P indices of every class)
+                tm.sync();                                  // the team's transposes have been read
 #pragma unroll
                 for (int j = 0; j < 16; ++j) xbuf[((tm.c * 16 + j) * 16 + tm.t) * CW] = v[j];
                 tm.sync();
@@ -235,7 +287,7 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
 #pragma unroll
                 for (int j = 0; j < 16; ++j) v[j] = xbuf[((tm.c * 16 + j) * 16 + tm.t) * CW];
             }
-            if constexpr (P == 1) tm.sync();                // transpose region: reads of the first transform are done
+            tm.sync();                                      // region free again for the transposes
             if constexpr (ROW) subline_fft<S2, CW>(v, sm_tw, ybuf, tm.t, hsync);
             else subline_fft<S2, CW>(v, sm_tw, ybuf, tm.t, tsync);
             cf *dst = line + tm.c * CS + tm.t * IS;
@@ -251,6 +303,8 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
     }
 }
 
+// Stage the pointwise factors of phase `d` for the unit this thread will work on, unless the
+// buffer already holds them.  Called while a grid barrier is pending.
 template <int P, int CW, bool ROW, int NX, int NY>
 __device__ __forceinline__ void prefill_phase16(const KParams &K, const Phase16 &d, cf *sm_pw, PwTag &tag) {
     typedef Team16<P, CW> TM;
@@ -274,29 +328,64 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const KParams P) {
     cf *sm_twcx = sm_tw + L::kTw;
     cf *sm_twcy = sm_twcx + (PX - 1) * kL;
     cf *sm_y = sm_twcy + (PY - 1) * kL;
-    cf *sm_x = sm_y + L::kY;
-    cf *sm_pw = sm_x + L::kX;
-    int *sm_abort = reinterpret_cast<int *>(sm_pw + L::kPw);
+    cf *sm_pwH = sm_y + L::kY;          // propagator values of this CTA's column tiles: stay put while the
+                                        // reference index (the table) does not change
+    cf *sm_pwS = sm_pwH + L::kPw;       // screen factors of this CTA's rows for the NEXT row phase
+    int *sm_abort = reinterpret_cast<int *>(sm_pwS + L::kPw);
 
     for (int i = threadIdx.x; i < L::kTw; i += kThreads16) sm_tw[i] = P.tw256[i];
     for (int i = threadIdx.x; i < (PX - 1) * kL; i += kThreads16) sm_twcx[i] = P.twcx[i];
     for (int i = threadIdx.x; i < (PY - 1) * kL; i += kThreads16) sm_twcy[i] = P.twcy[i];
     __syncthreads();
 
-    PwTag tag = {nullptr, -1};
+    PwTag tagH = {nullptr, -1}, tagS = {nullptr, -1};
     unsigned nbar = 0;
+    // optional timeline (bb_probe_trace): per phase and CTA, clock64 at phase start / work done /
+    // arrived / prefilled / released, and the global timer at release
+    long long *tr = P.trace ? P.trace + ((long long)(P.p0 - P.trace_p0) * gridDim.x + blockIdx.x) * 6 : nullptr;
+    const bool tracer = tr != nullptr && threadIdx.x == 0;
 #pragma unroll 1
     for (int p = P.p0; p < P.p1; ++p) {
         const Phase16 d = decode_phase16(P, p);
-        if (d.is_row) run_phase16<PX, 1, true, NX, NY>(P, d, sm_tw, sm_twcx, sm_y, sm_x, sm_pw, tag);
-        else run_phase16<PY, kCW16, false, NX, NY>(P, d, sm_tw, sm_twcy, sm_y, sm_x, sm_pw, tag);
+        if (tracer) tr[0] = clock64();
+        if (d.is_row && p + 2 < P.p1) {
+            // the dn rows this CTA turns into screen factors at the end of this phase (for the row
+            // phase after next): start them on their way from HBM to L2 now, one bulk prefetch per row
+            const int r0 = (int)(((long long)NY * blockIdx.x) / gridDim.x);
+            const int r1 = (int)(((long long)NY * (blockIdx.x + 1)) / gridDim.x);
+            if ((int)threadIdx.x < r1 - r0) {
+                const float *row = P.dn + (long long)((p >> 1) - P.j_base) * ((long long)NX * NY)
+                                   + (long long)(r0 + threadIdx.x) * NX;
+                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(row), "r"(NX * 4) : "memory");
+            }
+        }
+        if (d.is_row) run_phase16<PX, 1, true, NX, NY>(P, d, sm_tw, sm_twcx, sm_y, sm_pwS, tagS);
+        else run_phase16<PY, kCW16, false, NX, NY>(P, d, sm_tw, sm_twcy, sm_y, sm_pwH, tagH);
+        if (tracer) tr[1] = clock64();
         if (p + 1 < P.p1) {
             ++nbar;
             grid_arrive(P.bar);
-            const Phase16 dn = decode_phase16(P, p + 1);
-            if (dn.is_row) prefill_phase16<PX, 1, true, NX, NY>(P, dn, sm_pw, tag);
-            else prefill_phase16<PY, kCW16, false, NX, NY>(P, dn, sm_pw, tag);
+            if (tracer) tr[2] = clock64();
+            // While the barrier is pending, stage what does not depend on the field.  After a row
+            // phase: the propagator values of the coming column phase (only when the table changed)
+            // and the screen factors of the NEXT row phase (its dn slice is known), so that the
+            // sin/cos work has a whole barrier + column phase of slack.  After a column phase:
+            // the screen factors, if they are not there yet (first row phase of a launch).
+            if (d.is_row) {
+                prefill_phase16<PY, kCW16, false, NX, NY>(P, decode_phase16(P, p + 1), sm_pwH, tagH);
+                if (p + 2 < P.p1) prefill_phase16<PX, 1, true, NX, NY>(P, decode_phase16(P, p + 2), sm_pwS, tagS);
+            } else {
+                prefill_phase16<PX, 1, true, NX, NY>(P, decode_phase16(P, p + 1), sm_pwS, tagS);
+            }
+            if (tracer) tr[3] = clock64();
             if (grid_wait(P.bar, nbar * gridDim.x, P.status, sm_abort)) return;
+            if (tracer) {
+                tr[4] = clock64();
+                long long g;
+                asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g));
+                tr[5] = g;
+                tr += 6 * gridDim.x;
+            }
         }
     }
 }
