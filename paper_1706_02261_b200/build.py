@@ -58,8 +58,10 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
         obj = os.path.join(OBJ, "bb_inst_tx%d.o" % tx)
         jobs.append((obj, [nvcc, *NVCC_FLAGS, "-DBB_TX=%d" % tx, "-c", os.path.join(CSRC, "bb_inst.cu"), "-o", obj]))
     for px in PXS:
-        obj = os.path.join(OBJ, "bb_inst16_px%d.o" % px)
-        jobs.append((obj, [nvcc, *NVCC_FLAGS, "-DBB_PX=%d" % px, "-c", os.path.join(CSRC, "bb_inst16.cu"), "-o", obj]))
+        for cw in (4, 8):
+            obj = os.path.join(OBJ, "bb_inst16_px%d_cw%d.o" % (px, cw))
+            jobs.append((obj, [nvcc, *NVCC_FLAGS, "-DBB_PX=%d" % px, "-DBB_CW=%d" % cw, "-c",
+                               os.path.join(CSRC, "bb_inst16.cu"), "-o", obj]))
     obj_api = os.path.join(OBJ, "bb_api.o")
     jobs.append((obj_api, [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, "bb_api.cu"), "-o", obj_api]))
     obj_probe = os.path.join(OBJ, "bb_probe.o")

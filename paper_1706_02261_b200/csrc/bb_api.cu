@@ -76,6 +76,8 @@ struct Plan {
     size_t table_capacity = 0;
     const cf **d_htab = nullptr;   // per-step arrays
     float *d_phase = nullptr;
+    int *d_fmax = nullptr;         // per step: largest live |kx bin| (16-point-thread kernel)
+    int cw4 = 0;                   // column tiles of 4 columns for the propagation being enqueued
     int step_cap = 0;
     int grid = 0;                  // persistent grid size (<= SM count)
     int sm_count = 0;
@@ -180,10 +182,11 @@ int get_plan(int Nx, int Ny, Plan **out) {
 
 int ensure_steps(Plan *p, int Nz) {
     if (Nz <= p->step_cap) return BB_OK;
-    if (p->d_htab) { cudaFree((void *)p->d_htab); cudaFree(p->d_phase); p->d_htab = nullptr; p->d_phase = nullptr; }
+    if (p->d_htab) { cudaFree((void *)p->d_htab); cudaFree(p->d_phase); cudaFree(p->d_fmax); p->d_htab = nullptr; p->d_phase = nullptr; p->d_fmax = nullptr; }
     int cap = std::max(Nz, 1024);
     BB_CUDA(cudaMalloc((void **)&p->d_htab, (size_t)cap * sizeof(cf *)));
     BB_CUDA(cudaMalloc(&p->d_phase, (size_t)cap * sizeof(float)));
+    BB_CUDA(cudaMalloc(&p->d_fmax, (size_t)cap * sizeof(int)));
     p->step_cap = cap;
     return BB_OK;
 }
@@ -197,6 +200,46 @@ int build_table(Plan *p, const TableKey &k, cf *dst, cudaStream_t s) {
     ++g_launches;
     BB_CUDA(cudaGetLastError());
     return BB_OK;
+}
+
+// Largest |DFT bin| f of an N-point axis with pitch dx for which the propagator of wavenumber k can be
+// non-zero (bb.h step 2: s = k^2 - kx^2 - ky^2 > 0 needs kx^2 < k^2).  Conservative: a bin within
+// 1e-9 of the cut counts as live (a live column that is in fact all zero is only computed in vain).
+int live_fmax(int N, double dx, double k) {
+    const double lim = k * k * (1.0 + 1e-9);
+    int f = (int)std::floor(k * (double)N * dx / kTwoPi);
+    f = std::max(0, std::min(f, N / 2));
+    auto kx2 = [&](int g) { double kx = kTwoPi * (double)g / ((double)N * dx); return kx * kx; };
+    while (f < N / 2 && kx2(f + 1) < lim) ++f;
+    while (f > 0 && !(kx2(f) < lim)) --f;
+    return f;
+}
+
+// Number of live column tiles of width cw (the host copy of bb::LiveCols::total, bb_kernels16.cuh).
+int live_tiles(int N, int F, int cw) {
+    const int P = N / 256, L = 256, ntc = L / cw;
+    int n = 0;
+    for (int c = 0; c < P; ++c) {
+        int lo_cols = F >= c ? (F - c) / P + 1 : 0;
+        lo_cols = std::min(lo_cols, L);
+        int hs = std::min((N - F - c + P - 1) / P, L);
+        int a = (lo_cols + cw - 1) / cw, b = ntc - hs / cw;
+        if (a + b >= ntc) { a = ntc; b = 0; }
+        n += a + b;
+    }
+    return n;
+}
+
+// Tile width of the column phase for a whole propagation (it must not change between the launches of
+// one propagation): 4 columns when the live tiles then still fit one per SM, else 8.
+void choose_tile_width(Plan *p, int Nz, float dx, float lambda, float n0, const float *nref) {
+    p->cw4 = 0;
+    if (!p->k16) return;
+    double k0 = kTwoPi / (double)lambda;
+    int F = 0;
+    for (int j = 0; j < Nz; ++j) F = std::max(F, live_fmax(p->Nx, (double)dx, k0 * (double)(nref ? nref[j] : n0)));
+    if (getenv("BB_K16_CW")) { p->cw4 = atoi(getenv("BB_K16_CW")) == 4; return; }
+    p->cw4 = live_tiles(p->Nx, F, 4) <= p->grid;
 }
 
 constexpr int kTableCacheFull = -1;   // internal: every cached table belongs to the launch being assembled
@@ -279,9 +322,9 @@ int launch_steps(Plan *p, cf *field, const float *dn, float *inten, long long in
     P.mode = 0;
     P.twx = p->twx; P.twy = p->twy; P.bar = p->bar; P.status = p->status;
     P.tw256 = p->tw256; P.twcx = p->twcx; P.twcy = p->twcy;
+    P.fmax = p->d_fmax; P.cw4 = p->cw4; P.zeros = (const cf *)(p->status + 16);
     P.flags = flags & 3u;
     const bool k16 = use_k16(p, B);
-    { const char *e = getenv("BB_DBG"); P.dbg = e ? atoi(e) : 0; }
     if (g_trace && k16 && 2 * j1 + 1 <= g_trace_phases) { P.trace = g_trace; P.trace_p0 = 0; }
     auto launch = [&](bool coop) {
         return k16 ? bb::kernel16_launch(p->Nx, p->Ny, P, p->grid, coop, s)
@@ -309,6 +352,7 @@ int launch_steps(Plan *p, cf *field, const float *dn, float *inten, long long in
 // whose distinct propagator tables fit the cache together (normally all of it).
 int prepare_steps(Plan *p, int B, int Nz, int j0, float dx, float dz, float lambda, float n0, const float *nref,
                   cudaStream_t s, std::vector<const cf *> &h_tab, std::vector<float> &h_phase, int *j_done) {
+    std::vector<int> h_fmax(Nz);
     double k0 = kTwoPi / (double)lambda;
     unsigned long long protect = ++p->tick;
     const cf *last_ptr = nullptr;
@@ -326,6 +370,7 @@ int prepare_steps(Plan *p, int B, int Nz, int j0, float dx, float dz, float lamb
         }
         h_tab[j] = last_ptr;
         h_phase[j] = (float)(k0 * (double)dz * ((double)n0 - (double)nr));
+        h_fmax[j] = getenv("BB_K16_NOPRUNE") ? p->Nx / 2 : live_fmax(p->Nx, (double)dx, k0 * (double)nr);
     }
     *j_done = j;
     if (j == j0) return BB_OK;
@@ -334,6 +379,8 @@ int prepare_steps(Plan *p, int B, int Nz, int j0, float dx, float dz, float lamb
     BB_CUDA(cudaMemcpyAsync((void *)(p->d_htab + j0), h_tab.data() + j0, (size_t)(j - j0) * sizeof(cf *),
                             cudaMemcpyHostToDevice, s));
     BB_CUDA(cudaMemcpyAsync(p->d_phase + j0, h_phase.data() + j0, (size_t)(j - j0) * sizeof(float),
+                            cudaMemcpyHostToDevice, s));
+    BB_CUDA(cudaMemcpyAsync(p->d_fmax + j0, h_fmax.data() + j0, (size_t)(j - j0) * sizeof(int),
                             cudaMemcpyHostToDevice, s));
     return BB_OK;
 }
@@ -385,26 +432,31 @@ cudaError_t kernel_launch(int Nx, int Ny, const KParams &P, int grid, bool coop,
     BB_SWITCH_TX(launch, Ny / 32, P, grid, coop, s)
     return cudaErrorInvalidValue;
 }
-#define BB_SWITCH_PX(fn, ...)                           \
-    switch (Nx / 256) {                                 \
-        case 1: return inst16_1_##fn(__VA_ARGS__);      \
-        case 2: return inst16_2_##fn(__VA_ARGS__);      \
-        case 4: return inst16_4_##fn(__VA_ARGS__);      \
+#define BB_SWITCH_PX(cw, fn, ...)                             \
+    switch (Nx / 256) {                                       \
+        case 1: return inst16_1_cw##cw##_##fn(__VA_ARGS__);   \
+        case 2: return inst16_2_cw##cw##_##fn(__VA_ARGS__);   \
+        case 4: return inst16_4_cw##cw##_##fn(__VA_ARGS__);   \
     }
 bool kernel16_supports(int Nx, int Ny) {
     auto ok = [](int n) { return n == 256 || n == 512 || n == 1024; };
     return ok(Nx) && ok(Ny);
 }
 int kernel16_prepare(int Nx, int Ny) {
-    BB_SWITCH_PX(prepare, Ny / 256)
-    return (int)cudaErrorInvalidValue;
+    int rc = (int)cudaErrorInvalidValue;
+    { auto f = [&]() -> cudaError_t { BB_SWITCH_PX(8, prepare, Ny / 256) return cudaErrorInvalidValue; }; rc = (int)f(); }
+    if (rc) return rc;
+    auto g = [&]() -> cudaError_t { BB_SWITCH_PX(4, prepare, Ny / 256) return cudaErrorInvalidValue; };
+    return (int)g();
 }
 int kernel16_blocks_per_sm(int Nx, int Ny) {
-    BB_SWITCH_PX(blocks_per_sm, Ny / 256)
-    return 0;
+    auto f = [&]() -> int { BB_SWITCH_PX(8, blocks_per_sm, Ny / 256) return 0; };
+    auto g = [&]() -> int { BB_SWITCH_PX(4, blocks_per_sm, Ny / 256) return 0; };
+    return std::min(f(), g());
 }
 cudaError_t kernel16_launch(int Nx, int Ny, const KParams &P, int grid, bool coop, cudaStream_t s) {
-    BB_SWITCH_PX(launch, Ny / 256, P, grid, coop, s)
+    if (P.cw4) { BB_SWITCH_PX(4, launch, Ny / 256, P, grid, coop, s) }
+    else { BB_SWITCH_PX(8, launch, Ny / 256, P, grid, coop, s) }
     return cudaErrorInvalidValue;
 }
 }  // namespace bb
@@ -460,6 +512,7 @@ int bb_propagate_ex(void *field, const float *dn, int Nx, int Ny, int Nz, float 
     if (rc) return rc;
     cudaStream_t s = opts ? (cudaStream_t)opts->stream : (cudaStream_t)0;
     const float *nref = opts ? opts->nref : nullptr;
+    choose_tile_width(p, Nz, dx, lambda, n0, nref);
     std::vector<const cf *> h_tab(Nz);
     std::vector<float> h_phase(Nz);
     double k0 = kTwoPi / (double)lambda;
@@ -495,6 +548,7 @@ int bb_propagate_host(void *field_host, const float *dn_host, int Nx, int Ny, in
     rc = get_plan(Nx, Ny, &p);
     if (rc) return rc;
     const float *nref = opts ? opts->nref : nullptr;
+    choose_tile_width(p, Nz, dx, lambda, n0, nref);
     const size_t npx = (size_t)Nx * Ny;
     const bool per_field = (flags & BB_INTENSITY_PER_FIELD) != 0;
     const int IB = per_field ? B : 1;                        // intensity volumes

@@ -90,14 +90,79 @@ struct Team16 {
     __device__ __forceinline__ int q(int jp) const { return t + 16 * (P * jp + c); }
 };
 
+// Columns that can hold light.  The propagator is zero for kx^2 >= k^2 (bb.h step 2, evanescent
+// cut), so on an oversampled grid (dx < lambda / 2n) a band of kx columns is exactly zero after
+// every column phase: such columns are neither computed, stored nor loaded.  F = largest |DFT bin|
+// that may be non-zero (from the host, conservative).  Bookkeeping is per tile of `cw` adjacent
+// memory columns; in the kx-class-major layout class c holds bins P k' + c, whose live columns are
+// a low run k' <= (F - c) / P and a high run k' >= ceil((N - F - c) / P).
+template <int P>
+struct LiveCols {
+    int nlo[P], nhi[P], ntc;           // live tiles at the low / high end of each class, tiles per class
+    __device__ __forceinline__ LiveCols(int F, int N, int cw_log2) {   // tiles of 1 << cw_log2 columns
+        const int L = N / P, cw = 1 << cw_log2;
+        ntc = L >> cw_log2;
+#pragma unroll
+        for (int c = 0; c < P; ++c) {
+            int lo_cols = F >= c ? (F - c) / P + 1 : 0;
+            if (lo_cols > L) lo_cols = L;
+            int hs = (N - F - c + P - 1) / P;
+            if (hs > L) hs = L;
+            int a = (lo_cols + cw - 1) >> cw_log2, b = ntc - (hs >> cw_log2);
+            if (a + b >= ntc) { a = ntc; b = 0; }
+            nlo[c] = a; nhi[c] = b;
+        }
+    }
+    __device__ __forceinline__ int total() const {
+        int n = 0;
+#pragma unroll
+        for (int c = 0; c < P; ++c) n += nlo[c] + nhi[c];
+        return n;
+    }
+    // m-th live tile -> tile index in memory order
+    __device__ __forceinline__ int tile(int m) const {
+        int u = 0;
+#pragma unroll
+        for (int c = 0; c < P; ++c) {
+            const int n = nlo[c] + nhi[c];
+            if (m >= 0 && m < n) u = c * ntc + (m < nlo[c] ? m : ntc - n + m);
+            m -= n;
+        }
+        return u;
+    }
+};
+
+// Bit i set: sub-line element e0 + 16 i (e0 < 16) of kx class c sits in a live tile of 1 << cw_log2
+// columns (cw_log2 <= 4).  Same rule as LiveCols, for one class, in closed form: the live tiles are
+// tau < lo or tau >= hi with tau = (e0 + 16 i) >> cw_log2 = (i << (4 - cw_log2)) + (e0 >> cw_log2).
+template <int P>
+__device__ __forceinline__ unsigned live_mask16(int F, int N, int c, int e0, int cw_log2) {
+    const int L = N / P, cw = 1 << cw_log2, ntc = L >> cw_log2;
+    int lo_cols = F >= c ? (F - c) / P + 1 : 0;
+    if (lo_cols > L) lo_cols = L;
+    int hs = (N - F - c + P - 1) / P;
+    if (hs > L) hs = L;
+    int lo = (lo_cols + cw - 1) >> cw_log2, hi = hs >> cw_log2;
+    if (lo >= hi) return 0xFFFFu;
+    (void)ntc;
+    const int sh = 4 - cw_log2, t2 = e0 >> cw_log2, r = (1 << sh) - 1;
+    int nl = (lo - t2 + r) >> sh, nh = (hi - t2 + r) >> sh;        // i < nl or i >= nh
+    nl = nl < 0 ? 0 : (nl > 16 ? 16 : nl);
+    nh = nh < 0 ? 0 : (nh > 16 ? 16 : nh);
+    return (((1u << nl) - 1u) | ~((1u << nh) - 1u)) & 0xFFFFu;
+}
+
 struct HalfWarpSync {
     unsigned mask;
     __device__ __forceinline__ void operator()() const { __syncwarp(mask); }
 };
-template <class T>
-struct TeamSync {
-    const T &tm;
-    __device__ __forceinline__ void operator()() const { tm.sync(); }
+// The CW * 16 threads that share the transposes of one class of a column tile (whole warps).
+template <int THREADS>
+struct ClassSync {
+    int id;
+    __device__ __forceinline__ void operator()() const {
+        asm volatile("bar.sync %0, %1;" ::"r"(id), "n"(THREADS) : "memory");
+    }
 };
 
 // sin and cos of the phase-screen argument (bb.h step 4).  Arguments are k0 dz (n - n_ref), a
@@ -187,27 +252,42 @@ __device__ __forceinline__ void fill_pw16(int kind, const void *src, int unit, f
 // ----------------------------------------------------------------------------------------
 template <int P, int CW, bool ROW, int NX, int NY>
 __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, const cf *sm_tw, const cf *sm_twc,
-                                            cf *sm_y, cf *sm_pw, PwTag &tag) {
+                                            cf *sm_y, cf *sm_pw, PwTag &tag, int Fin, int Fout, int cwc) {
     typedef Team16<P, CW> TM;
     constexpr int S1 = ROW ? +1 : -1, S2 = -S1;
     constexpr int JP = TM::JP;
     constexpr long long NS = ROW ? 1 : NX;               // element stride of the line index
     constexpr long long CS = ROW ? kL : NX;              // class stride: class-major (rows) / interleaved (columns)
     constexpr long long IS = ROW ? 1 : (long long)P * NX;   // stride inside a class
-    constexpr int NU = ROW ? NY : NX / CW;
     const TM tm;
+    // rows: all of them; columns: the live tiles of this step (Fin), spread evenly over the CTAs
+    constexpr int CWL = CW == 8 ? 3 : (CW == 4 ? 2 : 0);
+    const LiveCols<ROW ? 1 : (NX / kL)> lv(Fin, NX, CWL);
+    const int NU = ROW ? NY : lv.total();
     const int a0 = (int)(((long long)NU * blockIdx.x) / gridDim.x);
     const int a1 = (int)(((long long)NU * (blockIdx.x + 1)) / gridDim.x);
+    // row phase: which of the thread's 16 sub-line elements sit in live column tiles on input (what
+    // the previous column phase wrote; the rest is stale and stands for zeros)
+    unsigned lmask = 0xFFFFu;
+    if constexpr (ROW) {
+        const int cwl = cwc == 4 ? 2 : 3;
+        lmask = live_mask16<P>(Fin, NX, tm.c, tm.t, cwl);
+    }
+    (void)Fout;
     cf *ybuf = sm_y + ((threadIdx.x / (16 * CW)) * (16 * 17 * CW)) + tm.col;        // one region per (team, class)
     cf *xbuf = sm_y + tm.team * (TM::TEAM * 17) + tm.col;                            // same memory, team's part
     cf *pw = sm_pw + threadIdx.x;
     const bool want_I = d.kind == 1 && K.inten != nullptr;
     const bool accumulate = (K.flags & 1u) != 0;
     const HalfWarpSync hsync{0xFFFFu << (16 * ((threadIdx.x >> 4) & 1))};
-    const TeamSync<TM> tsync{tm};
+    // hardware barriers: 0 = CTA, 1 .. NTEAM = teams, above = (team, class) groups of a column tile
+    // (one class: the class group is the team)
+    const ClassSync<16 * CW> tsync{P == 1 ? 1 + tm.team : 1 + TM::NTEAM + (int)threadIdx.x / (16 * CW)};
+    static_assert(ROW || ((16 * CW) % 32 == 0 && (P == 1 ? TM::NTEAM : TM::NTEAM + kThreads16 / (16 * CW)) <= 15), "barrier ids");
 
 #pragma unroll 1
-    for (int u = a0 + tm.team; u < a1; u += TM::NTEAM) {
+    for (int m = a0 + tm.team; m < a1; m += TM::NTEAM) {
+        const int u = ROW ? m : lv.tile(m);
         if (d.kind != 0 && (tag.src != d.src || tag.pix0 != u)) {
             fill_pw16<P, CW, ROW, NX>(d.kind, d.src, u, d.pa, K.phase_b, pw);
             tag.src = d.src; tag.pix0 = u;
@@ -217,7 +297,10 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
         if (d.first) {
             const cf *src = line + tm.c * CS + tm.t * IS;
 #pragma unroll
-            for (int i = 0; i < 16; ++i) v[i] = ld_cg(src + 16 * IS * i);
+            for (int i = 0; i < 16; ++i) {
+                v[i] = make_float2(0.f, 0.f);
+                if (!ROW || ((lmask >> i) & 1u)) v[i] = ld_cg(src + 16 * IS * i);
+            }
             if constexpr (ROW) subline_fft<S1, CW>(v, sm_tw, ybuf, tm.t, hsync);
             else subline_fft<S1, CW>(v, sm_tw, ybuf, tm.t, tsync);
             if constexpr (P > 1) {
@@ -292,7 +375,8 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
             else subline_fft<S2, CW>(v, sm_tw, ybuf, tm.t, tsync);
             cf *dst = line + tm.c * CS + tm.t * IS;
 #pragma unroll
-            for (int i = 0; i < 16; ++i) st_cg(dst + 16 * IS * i, v[i]);
+            for (int i = 0; i < 16; ++i) st_cg(dst + 16 * IS * i, v[i]);     // dead columns too: predicated
+                                                                              // stores cost more than they save
         } else {
 #pragma unroll
             for (int jp = 0; jp < JP; ++jp)
@@ -306,20 +390,23 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
 // Stage the pointwise factors of phase `d` for the unit this thread will work on, unless the
 // buffer already holds them.  Called while a grid barrier is pending.
 template <int P, int CW, bool ROW, int NX, int NY>
-__device__ __forceinline__ void prefill_phase16(const KParams &K, const Phase16 &d, cf *sm_pw, PwTag &tag) {
+__device__ __forceinline__ void prefill_phase16(const KParams &K, const Phase16 &d, cf *sm_pw, PwTag &tag, int Fin) {
     typedef Team16<P, CW> TM;
     if (d.kind == 0) return;
-    constexpr int NU = ROW ? NY : NX / CW;
     const TM tm;
+    const LiveCols<ROW ? 1 : (NX / kL)> lv(Fin, NX, CW == 8 ? 3 : (CW == 4 ? 2 : 0));
+    const int NU = ROW ? NY : lv.total();
     const int a0 = (int)(((long long)NU * blockIdx.x) / gridDim.x);
     const int a1 = (int)(((long long)NU * (blockIdx.x + 1)) / gridDim.x);
-    const int u = a0 + tm.team;
-    if (u >= a1 || (tag.src == d.src && tag.pix0 == u)) return;
+    const int m = a0 + tm.team;
+    if (m >= a1) return;
+    const int u = ROW ? m : lv.tile(m);
+    if (tag.src == d.src && tag.pix0 == u) return;
     fill_pw16<P, CW, ROW, NX>(d.kind, d.src, u, d.pa, K.phase_b, sm_pw + threadIdx.x);
     tag.src = d.src; tag.pix0 = u;
 }
 
-template <int PX, int PY>
+template <int PX, int PY, int CWC>     // CWC: columns per column tile (8, or 4 when few columns are live)
 __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const KParams P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     using L = Smem16<PX, PY>;
@@ -339,6 +426,17 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const KParams P) {
     __syncthreads();
 
     PwTag tagH = {nullptr, -1}, tagS = {nullptr, -1};
+    // largest live |kx bin| of the step whose column phase wrote (Fa) / will read (Fb) the field of a
+    // phase; fetched one phase ahead so that the global load is not on the critical path
+    auto live_in = [&](int p) {
+        const bool row = (p & 1) == 0;
+        return row ? ((p >> 1) >= 1 ? P.fmax[(p >> 1) - 1] : NX / 2) : P.fmax[p >> 1];
+    };
+    auto live_out = [&](int p) {
+        const bool row = (p & 1) == 0;
+        return row ? ((p >> 1) < P.Nz_total ? P.fmax[p >> 1] : NX / 2) : P.fmax[p >> 1];
+    };
+    int Fa_next = live_in(P.p0), Fb_next = live_out(P.p0);
     unsigned nbar = 0;
     // optional timeline (bb_probe_trace): per phase and CTA, clock64 at phase start / work done /
     // arrived / prefilled / released, and the global timer at release
@@ -359,23 +457,28 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const KParams P) {
                 asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(row), "r"(NX * 4) : "memory");
             }
         }
-        if (d.is_row) run_phase16<PX, 1, true, NX, NY>(P, d, sm_tw, sm_twcx, sm_y, sm_pwS, tagS);
-        else run_phase16<PY, kCW16, false, NX, NY>(P, d, sm_tw, sm_twcy, sm_y, sm_pwH, tagH);
+        // largest live |kx bin| of the step whose column phase wrote / will read the field
+        const int Fa = Fa_next, Fb = Fb_next;
+        if (d.is_row) run_phase16<PX, 1, true, NX, NY>(P, d, sm_tw, sm_twcx, sm_y, sm_pwS, tagS, Fa, Fb, CWC);
+        else run_phase16<PY, CWC, false, NX, NY>(P, d, sm_tw, sm_twcy, sm_y, sm_pwH, tagH, Fa, Fa, CWC);
         if (tracer) tr[1] = clock64();
         if (p + 1 < P.p1) {
             ++nbar;
             grid_arrive(P.bar);
             if (tracer) tr[2] = clock64();
+            Fa_next = live_in(p + 1);
+            Fb_next = live_out(p + 1);
             // While the barrier is pending, stage what does not depend on the field.  After a row
             // phase: the propagator values of the coming column phase (only when the table changed)
             // and the screen factors of the NEXT row phase (its dn slice is known), so that the
             // sin/cos work has a whole barrier + column phase of slack.  After a column phase:
             // the screen factors, if they are not there yet (first row phase of a launch).
             if (d.is_row) {
-                prefill_phase16<PY, kCW16, false, NX, NY>(P, decode_phase16(P, p + 1), sm_pwH, tagH);
-                if (p + 2 < P.p1) prefill_phase16<PX, 1, true, NX, NY>(P, decode_phase16(P, p + 2), sm_pwS, tagS);
+                const int Fn = P.fmax[(p + 1) >> 1];
+                prefill_phase16<PY, CWC, false, NX, NY>(P, decode_phase16(P, p + 1), sm_pwH, tagH, Fn);
+                if (p + 2 < P.p1) prefill_phase16<PX, 1, true, NX, NY>(P, decode_phase16(P, p + 2), sm_pwS, tagS, 0);
             } else {
-                prefill_phase16<PX, 1, true, NX, NY>(P, decode_phase16(P, p + 1), sm_pwS, tagS);
+                prefill_phase16<PX, 1, true, NX, NY>(P, decode_phase16(P, p + 1), sm_pwS, tagS, 0);
             }
             if (tracer) tr[3] = clock64();
             if (grid_wait(P.bar, nbar * gridDim.x, P.status, sm_abort)) return;

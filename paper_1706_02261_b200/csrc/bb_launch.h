@@ -18,14 +18,18 @@ BB_DECLARE_INST(16)
 BB_DECLARE_INST(32)
 #undef BB_DECLARE_INST
 
-// 16-point-thread kernel (bb_kernels16.cuh), one set per PX = Nx/256 in {1, 2, 4}; bb_inst16.cu.
-#define BB_DECLARE_INST16(PX)                                                                      \
-    cudaError_t inst16_##PX##_prepare(int PY);                                                     \
-    int inst16_##PX##_blocks_per_sm(int PY);                                                       \
-    cudaError_t inst16_##PX##_launch(int PY, const KParams &P, int grid, bool coop, cudaStream_t s);
-BB_DECLARE_INST16(1)
-BB_DECLARE_INST16(2)
-BB_DECLARE_INST16(4)
+// 16-point-thread kernel (bb_kernels16.cuh), one set per PX = Nx/256 in {1, 2, 4} and column
+// tile width in {4, 8}; bb_inst16.cu.
+#define BB_DECLARE_INST16(PX, CW)                                                                          \
+    cudaError_t inst16_##PX##_cw##CW##_prepare(int PY);                                                     \
+    int inst16_##PX##_cw##CW##_blocks_per_sm(int PY);                                                       \
+    cudaError_t inst16_##PX##_cw##CW##_launch(int PY, const KParams &P, int grid, bool coop, cudaStream_t s);
+BB_DECLARE_INST16(1, 4)
+BB_DECLARE_INST16(2, 4)
+BB_DECLARE_INST16(4, 4)
+BB_DECLARE_INST16(1, 8)
+BB_DECLARE_INST16(2, 8)
+BB_DECLARE_INST16(4, 8)
 #undef BB_DECLARE_INST16
 
 // Dispatch on (Nx, Ny); defined in bb_api.cu.

@@ -67,6 +67,28 @@ def test_small_shapes_batches_and_ragged_tiles(oracle_mod, Nx, Ny, Nz, B):
     assert not np.isnan(I).any()
 
 
+@pytest.mark.parametrize("Nx,Ny,dx,nlo,nhi", [(256, 256, 0.05, 1.2, 1.5), (512, 256, 0.07, 1.0, 1.6),
+                                              (1024, 512, 0.1, 1.3, 1.4), (1024, 1024, 0.06, 1.33, 1.38),
+                                              (256, 1024, 0.12, 1.1, 1.9), (512, 512, 0.2, 1.33, 1.36)])
+def test_oversampled_grids_skip_the_evanescent_band(oracle_mod, Nx, Ny, dx, nlo, nhi):
+    """dx < lambda / 2n: a band of kx columns is evanescent and the 16-point-thread kernel neither
+    computes nor reads it.  The reference index changes at every
+    step, so the band edge moves between steps; the dead columns of the field buffer keep stale
+    values (first the input field itself) that must not leak into the result."""
+    bb = need_gpu()
+    Nz = 7
+    w = wl.tiny(N=Nx, Nz=Nz, n_cells=10, r_lo=0.5, r_hi=3.0)
+    w = wl.dataclasses.replace(w, Ny=Ny, dx=dx)
+    dn = wl.make_dn(w)
+    f0 = wl.random_field(Nx, Ny, seed=3 * Nx + Ny, batch=1)
+    nref = np.linspace(nlo, nhi, Nz).astype(np.float32)
+    nref[1::2] = nref[1::2][::-1].copy()                     # not monotone either
+    u, I, uo, Io = run_both(bb, oracle_mod, w, dn, f0, nref)
+    assert rel_l2(u[0], uo[0]) < small_tol(Nz)
+    assert rel_l2(I, Io) < 2 * small_tol(Nz)
+    assert np.isfinite(I).all() and np.isfinite(u).all()
+
+
 @pytest.mark.parametrize("flags", ["per_field", "accumulate", "per_field+accumulate", "per_phase"])
 def test_flags(oracle_mod, flags):
     bb = need_gpu()
