@@ -59,9 +59,10 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
         jobs.append((obj, [nvcc, *NVCC_FLAGS, "-DBB_TX=%d" % tx, "-c", os.path.join(CSRC, "bb_inst.cu"), "-o", obj]))
     for px in PXS:
         for cw in (4, 8):
-            obj = os.path.join(OBJ, "bb_inst16_px%d_cw%d.o" % (px, cw))
-            jobs.append((obj, [nvcc, *NVCC_FLAGS, "-DBB_PX=%d" % px, "-DBB_CW=%d" % cw, "-c",
-                               os.path.join(CSRC, "bb_inst16.cu"), "-o", obj]))
+            for bt in (0, 1):
+                obj = os.path.join(OBJ, "bb_inst16_px%d_cw%d_b%d.o" % (px, cw, bt))
+                jobs.append((obj, [nvcc, *NVCC_FLAGS, "-DBB_PX=%d" % px, "-DBB_CW=%d" % cw, "-DBB_BATCH=%d" % bt, "-c",
+                                   os.path.join(CSRC, "bb_inst16.cu"), "-o", obj]))
     obj_api = os.path.join(OBJ, "bb_api.o")
     jobs.append((obj_api, [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, "bb_api.cu"), "-o", obj_api]))
     obj_probe = os.path.join(OBJ, "bb_probe.o")

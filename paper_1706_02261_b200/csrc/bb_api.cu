@@ -231,15 +231,15 @@ int live_tiles(int N, int F, int cw) {
 }
 
 // Tile width of the column phase for a whole propagation (it must not change between the launches of
-// one propagation): 4 columns when the live tiles then still fit one per SM, else 8.
-void choose_tile_width(Plan *p, int Nz, float dx, float lambda, float n0, const float *nref) {
+// one propagation): 4 columns when the (tile, field) units then still fit one per SM, else 8.
+void choose_tile_width(Plan *p, int B, int Nz, float dx, float lambda, float n0, const float *nref) {
     p->cw4 = 0;
     if (!p->k16) return;
     double k0 = kTwoPi / (double)lambda;
     int F = 0;
     for (int j = 0; j < Nz; ++j) F = std::max(F, live_fmax(p->Nx, (double)dx, k0 * (double)(nref ? nref[j] : n0)));
     if (getenv("BB_K16_CW")) { p->cw4 = atoi(getenv("BB_K16_CW")) == 4; return; }
-    p->cw4 = live_tiles(p->Nx, F, 4) <= p->grid;
+    p->cw4 = live_tiles(p->Nx, F, 4) * B <= p->grid;
 }
 
 constexpr int kTableCacheFull = -1;   // internal: every cached table belongs to the launch being assembled
@@ -301,7 +301,12 @@ int validate_common(const void *field, const float *dn, int Nx, int Ny, int Nz, 
 
 // The 16-point-thread kernel serves single fields on 256/512/1024 grids; everything else (batches,
 // other shapes, the generic transform programs) runs on the 32-point-thread kernel.
-bool use_k16(const Plan *p, int B) { return p->k16 && B == 1; }
+bool use_k16(const Plan *p, int B) {
+    if (!p->k16) return false;
+    // the batch variant shares one buffer of screen factors among the teams: all rows of a CTA must fit
+    const int rows = (p->Ny + p->grid - 1) / p->grid;
+    return B == 1 || (long long)rows * p->Nx <= 8192;
+}
 
 int batch_warps(int B) {
     int bw = 1;
@@ -432,31 +437,42 @@ cudaError_t kernel_launch(int Nx, int Ny, const KParams &P, int grid, bool coop,
     BB_SWITCH_TX(launch, Ny / 32, P, grid, coop, s)
     return cudaErrorInvalidValue;
 }
-#define BB_SWITCH_PX(cw, fn, ...)                             \
-    switch (Nx / 256) {                                       \
-        case 1: return inst16_1_cw##cw##_##fn(__VA_ARGS__);   \
-        case 2: return inst16_2_cw##cw##_##fn(__VA_ARGS__);   \
-        case 4: return inst16_4_cw##cw##_##fn(__VA_ARGS__);   \
+#define BB_SWITCH_PX(cw, bt, fn, ...)                                 \
+    switch (Nx / 256) {                                               \
+        case 1: return inst16_1_cw##cw##_b##bt##_##fn(__VA_ARGS__);   \
+        case 2: return inst16_2_cw##cw##_b##bt##_##fn(__VA_ARGS__);   \
+        case 4: return inst16_4_cw##cw##_b##bt##_##fn(__VA_ARGS__);   \
     }
 bool kernel16_supports(int Nx, int Ny) {
     auto ok = [](int n) { return n == 256 || n == 512 || n == 1024; };
     return ok(Nx) && ok(Ny);
 }
 int kernel16_prepare(int Nx, int Ny) {
-    int rc = (int)cudaErrorInvalidValue;
-    { auto f = [&]() -> cudaError_t { BB_SWITCH_PX(8, prepare, Ny / 256) return cudaErrorInvalidValue; }; rc = (int)f(); }
-    if (rc) return rc;
-    auto g = [&]() -> cudaError_t { BB_SWITCH_PX(4, prepare, Ny / 256) return cudaErrorInvalidValue; };
-    return (int)g();
+    auto f0 = [&]() -> cudaError_t { BB_SWITCH_PX(8, 0, prepare, Ny / 256) return cudaErrorInvalidValue; };
+    auto f1 = [&]() -> cudaError_t { BB_SWITCH_PX(4, 0, prepare, Ny / 256) return cudaErrorInvalidValue; };
+    auto f2 = [&]() -> cudaError_t { BB_SWITCH_PX(8, 1, prepare, Ny / 256) return cudaErrorInvalidValue; };
+    auto f3 = [&]() -> cudaError_t { BB_SWITCH_PX(4, 1, prepare, Ny / 256) return cudaErrorInvalidValue; };
+    cudaError_t e = f0();
+    if (e == cudaSuccess) e = f1();
+    if (e == cudaSuccess) e = f2();
+    if (e == cudaSuccess) e = f3();
+    return (int)e;
 }
 int kernel16_blocks_per_sm(int Nx, int Ny) {
-    auto f = [&]() -> int { BB_SWITCH_PX(8, blocks_per_sm, Ny / 256) return 0; };
-    auto g = [&]() -> int { BB_SWITCH_PX(4, blocks_per_sm, Ny / 256) return 0; };
-    return std::min(f(), g());
+    auto f0 = [&]() -> int { BB_SWITCH_PX(8, 0, blocks_per_sm, Ny / 256) return 0; };
+    auto f1 = [&]() -> int { BB_SWITCH_PX(4, 0, blocks_per_sm, Ny / 256) return 0; };
+    auto f2 = [&]() -> int { BB_SWITCH_PX(8, 1, blocks_per_sm, Ny / 256) return 0; };
+    auto f3 = [&]() -> int { BB_SWITCH_PX(4, 1, blocks_per_sm, Ny / 256) return 0; };
+    return std::min(std::min(f0(), f1()), std::min(f2(), f3()));
 }
 cudaError_t kernel16_launch(int Nx, int Ny, const KParams &P, int grid, bool coop, cudaStream_t s) {
-    if (P.cw4) { BB_SWITCH_PX(4, launch, Ny / 256, P, grid, coop, s) }
-    else { BB_SWITCH_PX(8, launch, Ny / 256, P, grid, coop, s) }
+    if (P.B > 1) {
+        if (P.cw4) { BB_SWITCH_PX(4, 1, launch, Ny / 256, P, grid, coop, s) }
+        else { BB_SWITCH_PX(8, 1, launch, Ny / 256, P, grid, coop, s) }
+    } else {
+        if (P.cw4) { BB_SWITCH_PX(4, 0, launch, Ny / 256, P, grid, coop, s) }
+        else { BB_SWITCH_PX(8, 0, launch, Ny / 256, P, grid, coop, s) }
+    }
     return cudaErrorInvalidValue;
 }
 }  // namespace bb
@@ -512,7 +528,7 @@ int bb_propagate_ex(void *field, const float *dn, int Nx, int Ny, int Nz, float 
     if (rc) return rc;
     cudaStream_t s = opts ? (cudaStream_t)opts->stream : (cudaStream_t)0;
     const float *nref = opts ? opts->nref : nullptr;
-    choose_tile_width(p, Nz, dx, lambda, n0, nref);
+    choose_tile_width(p, B, Nz, dx, lambda, n0, nref);
     std::vector<const cf *> h_tab(Nz);
     std::vector<float> h_phase(Nz);
     double k0 = kTwoPi / (double)lambda;
@@ -548,7 +564,7 @@ int bb_propagate_host(void *field_host, const float *dn_host, int Nx, int Ny, in
     rc = get_plan(Nx, Ny, &p);
     if (rc) return rc;
     const float *nref = opts ? opts->nref : nullptr;
-    choose_tile_width(p, Nz, dx, lambda, n0, nref);
+    choose_tile_width(p, B, Nz, dx, lambda, n0, nref);
     const size_t npx = (size_t)Nx * Ny;
     const bool per_field = (flags & BB_INTENSITY_PER_FIELD) != 0;
     const int IB = per_field ? B : 1;                        // intensity volumes

@@ -1,4 +1,4 @@
-// bb_kernels16.cuh -- the BPM step kernel with 16 points per thread (Nx, Ny in {256, 512, 1024}, B = 1).
+// bb_kernels16.cuh -- the BPM step kernel with 16 points per thread (Nx, Ny in {256, 512, 1024}; single fields and batches).
 //
 // Same two-phase structure as bb_kernels.cuh:
 //   column phase C_j : FFT_y  -> x H_j                          -> IFFT_y
@@ -246,11 +246,30 @@ __device__ __forceinline__ void fill_pw16(int kind, const void *src, int unit, f
     }
 }
 
+// Batch kernel: screen factors of ALL rows this CTA owns, pw[rl * NX + n] = exp(i (pb dn + pa)) at
+// pixel n of row a0 + rl, staged by the whole CTA (coalesced dn reads) and shared by the teams that
+// apply them to the B fields.
+template <int NX, int NY>
+__device__ __forceinline__ void stage_rows_screen(const KParams &K, const Phase16 &d, cf *pw) {
+    const int a0 = (int)(((long long)NY * blockIdx.x) / gridDim.x);
+    const int a1 = (int)(((long long)NY * (blockIdx.x + 1)) / gridDim.x);
+    const int total = (a1 - a0) * NX;
+    const float *dnp = reinterpret_cast<const float *>(d.src) + (long long)a0 * NX;
+#pragma unroll 4
+    for (int idx = threadIdx.x; idx < total; idx += kThreads16) {
+        const float a = fmaf(K.phase_b, __ldcs(dnp + idx), d.pa);
+        float s, c;
+        if (__all_sync(__activemask(), fabsf(a) <= 0.78539816f)) screen_sincos_small(a, s, c);
+        else screen_sincos(a, s, c);
+        pw[idx] = make_float2(c, s);
+    }
+}
+
 // ----------------------------------------------------------------------------------------
 // One phase over the lines (rows, or tiles of CW columns) this CTA owns.
 //   ROW : P = PX, CW = 1, signs (+1, -1);  column: P = PY, CW = kCW16, signs (-1, +1).
 // ----------------------------------------------------------------------------------------
-template <int P, int CW, bool ROW, int NX, int NY>
+template <int P, int CW, bool ROW, int NX, int NY, bool BATCH>
 __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, const cf *sm_tw, const cf *sm_twc,
                                             cf *sm_y, cf *sm_pw, PwTag &tag, int Fin, int Fout, int cwc) {
     typedef Team16<P, CW> TM;
@@ -279,6 +298,24 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
     cf *pw = sm_pw + threadIdx.x;
     const bool want_I = d.kind == 1 && K.inten != nullptr;
     const bool accumulate = (K.flags & 1u) != 0;
+    // batch kernel: units are (line, field) pairs, fields fastest, so that the teams of a CTA share
+    // the pointwise factors of a line; the summed intensity of a row is accumulated in shared
+    // memory (acc, floats, in the buffer the propagator values use during column phases)
+    const int B = BATCH ? K.B : 1;
+    const long long npx = (long long)NX * NY;
+    const bool summed = BATCH && ROW && want_I && !(K.flags & 2u) && K.B > 1;
+    float *acc = reinterpret_cast<float *>(sm_pw - Smem16<NX / kL, NY / kL>::kPw);   // = the H buffer (ROW: sm_pw is the screen buffer)
+    if constexpr (BATCH && ROW) {
+        if (d.kind == 1 && tag.src != d.src) {                 // CTA-uniform: not staged during the barrier
+            stage_rows_screen<NX, NY>(K, d, sm_pw);
+            tag.src = d.src;
+            __syncthreads();
+        }
+        if (summed) {
+            for (int idx = threadIdx.x; idx < (a1 - a0) * NX; idx += kThreads16) acc[idx] = 0.f;
+            __syncthreads();
+        }
+    }
     const HalfWarpSync hsync{0xFFFFu << (16 * ((threadIdx.x >> 4) & 1))};
     // hardware barriers: 0 = CTA, 1 .. NTEAM = teams, above = (team, class) groups of a column tile
     // (one class: the class group is the team)
@@ -286,13 +323,18 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
     static_assert(ROW || ((16 * CW) % 32 == 0 && (P == 1 ? TM::NTEAM : TM::NTEAM + kThreads16 / (16 * CW)) <= 15), "barrier ids");
 
 #pragma unroll 1
-    for (int m = a0 + tm.team; m < a1; m += TM::NTEAM) {
+    const int k0 = BATCH ? (ROW ? a0 * B : (int)(((long long)NU * B * blockIdx.x) / gridDim.x)) : a0;
+    const int k1 = BATCH ? (ROW ? a1 * B : (int)(((long long)NU * B * (blockIdx.x + 1)) / gridDim.x)) : a1;
+    for (int k = k0 + tm.team; k < k1; k += TM::NTEAM) {
+        const int m = BATCH ? k / B : k, b = BATCH ? k - m * B : 0;
         const int u = ROW ? m : lv.tile(m);
-        if (d.kind != 0 && (tag.src != d.src || tag.pix0 != u)) {
+        if constexpr (BATCH && ROW) {
+            pw = sm_pw + (m - a0) * NX;                         // the row's factors, indexed by pixel
+        } else if (d.kind != 0 && (tag.src != d.src || tag.pix0 != u)) {
             fill_pw16<P, CW, ROW, NX>(d.kind, d.src, u, d.pa, K.phase_b, pw);
             tag.src = d.src; tag.pix0 = u;
         }
-        cf *line = K.field + (ROW ? (long long)u * NX : (long long)u * CW + tm.col);
+        cf *line = K.field + b * npx + (ROW ? (long long)u * NX : (long long)u * CW + tm.col);
         cf v[16];
         if (d.first) {
             const cf *src = line + tm.c * CS + tm.t * IS;
@@ -331,17 +373,34 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
         // v[jp*P + m] is element n = q(jp) + 256 m of the line, in its natural (x- or ky-) order
         if (d.kind == 1) {
             // u = value * screen (bb.h step 4), intensity (step 5)
-#pragma unroll
-            for (int i = 0; i < 16; ++i) v[i] = cmul(v[i], pw[i * kThreads16]);
-            if (want_I) {
-                float *ip = K.inten + d.slice + (long long)u * NX;
+            if constexpr (BATCH) {
 #pragma unroll
                 for (int jp = 0; jp < JP; ++jp)
 #pragma unroll
-                    for (int m = 0; m < P; ++m) {
-                        const cf w = v[jp * P + m];
+                    for (int mm = 0; mm < P; ++mm) v[jp * P + mm] = cmul(v[jp * P + mm], pw[tm.q(jp) + kL * mm]);
+            } else {
+#pragma unroll
+                for (int i = 0; i < 16; ++i) v[i] = cmul(v[i], pw[i * kThreads16]);
+            }
+            if (summed) {
+                float *ar = acc + (m - a0) * NX;
+#pragma unroll
+                for (int jp = 0; jp < JP; ++jp)
+#pragma unroll
+                    for (int mm = 0; mm < P; ++mm) {
+                        const cf w = v[jp * P + mm];
+                        atomicAdd(ar + tm.q(jp) + kL * mm, fmaf(w.x, w.x, w.y * w.y));
+                    }
+            } else if (want_I) {
+                float *ip = K.inten + d.slice + (long long)u * NX
+                            + ((K.flags & 2u) ? (long long)b * K.inten_bstride : 0);
+#pragma unroll
+                for (int jp = 0; jp < JP; ++jp)
+#pragma unroll
+                    for (int mm = 0; mm < P; ++mm) {
+                        const cf w = v[jp * P + mm];
                         float I = fmaf(w.x, w.x, w.y * w.y);
-                        float *a = ip + tm.q(jp) + kL * m;
+                        float *a = ip + tm.q(jp) + kL * mm;
                         if (accumulate) I += *a;
                         __stcs(a, I);
                     }
@@ -385,28 +444,52 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
         }
         tm.sync();                                          // buffers free for the team's next unit
     }
+    if constexpr (BATCH && ROW) {
+        if (summed) {
+            // I[j] (+)= sum over the fields (bb.h step 5): the CTA's rows are contiguous in the slice
+            __syncthreads();
+            float *ip = K.inten + d.slice + (long long)a0 * NX;
+            for (int idx = threadIdx.x; idx < (a1 - a0) * NX; idx += kThreads16) {
+                float I = acc[idx];
+                if (accumulate) I += ip[idx];
+                __stcs(ip + idx, I);
+            }
+        }
+    }
 }
 
 // Stage the pointwise factors of phase `d` for the unit this thread will work on, unless the
 // buffer already holds them.  Called while a grid barrier is pending.
-template <int P, int CW, bool ROW, int NX, int NY>
+template <int P, int CW, bool ROW, int NX, int NY, bool BATCH>
 __device__ __forceinline__ void prefill_phase16(const KParams &K, const Phase16 &d, cf *sm_pw, PwTag &tag, int Fin) {
     typedef Team16<P, CW> TM;
     if (d.kind == 0) return;
+    if constexpr (BATCH && ROW) {
+        if (tag.src != d.src) {
+            stage_rows_screen<NX, NY>(K, d, sm_pw);
+            tag.src = d.src;
+        }
+        return;
+    }
     const TM tm;
     const LiveCols<ROW ? 1 : (NX / kL)> lv(Fin, NX, CW == 8 ? 3 : (CW == 4 ? 2 : 0));
     const int NU = ROW ? NY : lv.total();
     const int a0 = (int)(((long long)NU * blockIdx.x) / gridDim.x);
     const int a1 = (int)(((long long)NU * (blockIdx.x + 1)) / gridDim.x);
-    const int m = a0 + tm.team;
-    if (m >= a1) return;
+    const int B = BATCH ? K.B : 1;
+    const int k0 = BATCH ? (int)(((long long)NU * B * blockIdx.x) / gridDim.x) : a0;
+    const int k1 = BATCH ? (int)(((long long)NU * B * (blockIdx.x + 1)) / gridDim.x) : a1;
+    const int k = k0 + tm.team;
+    if (k >= k1) return;
+    const int m = BATCH ? k / B : k;
     const int u = ROW ? m : lv.tile(m);
     if (tag.src == d.src && tag.pix0 == u) return;
     fill_pw16<P, CW, ROW, NX>(d.kind, d.src, u, d.pa, K.phase_b, sm_pw + threadIdx.x);
     tag.src = d.src; tag.pix0 = u;
 }
 
-template <int PX, int PY, int CWC>     // CWC: columns per column tile (8, or 4 when few columns are live)
+// CWC: columns per column tile (8, or 4 when few columns are live); BATCH: several fields (KParams::B)
+template <int PX, int PY, int CWC, bool BATCH>
 __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const KParams P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     using L = Smem16<PX, PY>;
@@ -459,9 +542,11 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const KParams P) {
         }
         // largest live |kx bin| of the step whose column phase wrote / will read the field
         const int Fa = Fa_next, Fb = Fb_next;
-        if (d.is_row) run_phase16<PX, 1, true, NX, NY>(P, d, sm_tw, sm_twcx, sm_y, sm_pwS, tagS, Fa, Fb, CWC);
-        else run_phase16<PY, CWC, false, NX, NY>(P, d, sm_tw, sm_twcy, sm_y, sm_pwH, tagH, Fa, Fa, CWC);
+        if (d.is_row) run_phase16<PX, 1, true, NX, NY, BATCH>(P, d, sm_tw, sm_twcx, sm_y, sm_pwS, tagS, Fa, Fb, CWC);
+        else run_phase16<PY, CWC, false, NX, NY, BATCH>(P, d, sm_tw, sm_twcy, sm_y, sm_pwH, tagH, Fa, Fa, CWC);
         if (tracer) tr[1] = clock64();
+        if (BATCH && d.is_row && d.kind == 1 && P.inten != nullptr && !(P.flags & 2u) && P.B > 1)
+            tagH.src = nullptr;                // the intensity sums used the propagator buffer
         if (p + 1 < P.p1) {
             ++nbar;
             grid_arrive(P.bar);
@@ -475,10 +560,10 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const KParams P) {
             // the screen factors, if they are not there yet (first row phase of a launch).
             if (d.is_row) {
                 const int Fn = P.fmax[(p + 1) >> 1];
-                prefill_phase16<PY, CWC, false, NX, NY>(P, decode_phase16(P, p + 1), sm_pwH, tagH, Fn);
-                if (p + 2 < P.p1) prefill_phase16<PX, 1, true, NX, NY>(P, decode_phase16(P, p + 2), sm_pwS, tagS, 0);
+                prefill_phase16<PY, CWC, false, NX, NY, BATCH>(P, decode_phase16(P, p + 1), sm_pwH, tagH, Fn);
+                if (p + 2 < P.p1) prefill_phase16<PX, 1, true, NX, NY, BATCH>(P, decode_phase16(P, p + 2), sm_pwS, tagS, 0);
             } else {
-                prefill_phase16<PX, 1, true, NX, NY>(P, decode_phase16(P, p + 1), sm_pwS, tagS, 0);
+                prefill_phase16<PX, 1, true, NX, NY, BATCH>(P, decode_phase16(P, p + 1), sm_pwS, tagS, 0);
             }
             if (tracer) tr[3] = clock64();
             if (grid_wait(P.bar, nbar * gridDim.x, P.status, sm_abort)) return;
