@@ -214,7 +214,7 @@ def run_ours(args):
     if clocks is not None:
         result["clocks"] = clocks
 
-    # ---- roofline of the dominant kernel (bb::bpm_kernel, one launch per propagation) ----
+    # ---- roofline of the dominant kernel (the persistent BPM kernel, one launch per propagation) ----
     hbm_b, l2_b, flop = algorithmic_per_step(w)
     hbm_peak, hbm_src = measured_peaks()
     dur = prop_ms * 1e-3
@@ -222,7 +222,7 @@ def run_ours(args):
     alu_ach = flop * w.Nz / dur / 1e12
     result["roofline"] = {"bound": "alu", "achieved": alu_ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
                           "frac": alu_ach / FP32_PEAK_TFLOPS, "traffic": traffic,
-                          "kernel": "bb::bpm_kernel", "peak_source": "nominal 148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md)",
+                          "kernel": "bb::bpm16_kernel<4,4,4,false>" if (w.Nx, w.Ny, B) == (1024, 1024, 1) else "bb::bpm_kernel / bb::bpm16_kernel", "peak_source": "nominal 148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md)",
                           "algorithmic_flop_per_launch": flop * w.Nz}
     hbm_ach = hbm_b * w.Nz / dur / 1e9
     result["roofline_hbm"] = {"bound": "hbm", "achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s",
@@ -242,6 +242,13 @@ def run_ours(args):
             result["hbm_l2_roofline_frac"] = t_roof / (dur / w.Nz)       # T_roof / T_measured per slice
         except Exception as e:                                            # noqa: BLE001
             result["roofline_l2"] = {"error": str(e)}
+
+    # ---- the batched workload (BASELINE.json configs[4]) beside the headline, for information ----
+    if rank == 0 and world == 1 and args.workload == "C4" and not args.nz and not args.no_batch:
+        try:
+            result["batch_workload"] = time_batch_workload(bb, dev)
+        except Exception as e:                                            # noqa: BLE001
+            result["batch_workload"] = {"error": str(e)}
 
     # ---- end to end through the host-buffer entry point ----
     if not args.no_e2e:
@@ -291,6 +298,29 @@ def run_ours(args):
     if rank == 0:
         print(json.dumps(result))
     replicas.shutdown()
+
+
+def time_batch_workload(bb, dev, steps=3):
+    """C5: 16 fields of 512x512 through a shared 512^3 volume, summed intensity (device-resident)."""
+    w = wl.config("C5")
+    dn, f0, _ = make_inputs(w, dev)
+    nref = bb.nref_from_dn(dn, w.n0, w.nref_slab).numpy()
+    f0_d = torch.from_numpy(f0).to(dev)
+    field = torch.empty_like(f0_d)
+    inten = torch.empty((w.Nz, w.Ny, w.Nx), dtype=torch.float32, device=dev)
+    ts = []
+    for i in range(steps + 2):
+        field.copy_(f0_d)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        bb.propagate(field, dn, w.dx, w.dz, w.lam, w.n0, intensity=inten, nref=nref)
+        b.record()
+        torch.cuda.synchronize()
+        if i >= 2:
+            ts.append(a.elapsed_time(b))
+    ms = statistics.mean(ts)
+    return {"workload": "C5: %d fields of %dx%d, %d z-slices, one shared dn volume, summed intensity" % (w.batch, w.Nx, w.Ny, w.Nz),
+            "propagate_ms": ms, "value": w.batch * w.Nx * w.Ny * w.Nz / (ms * 1e-3) / 1e6, "unit": "Mvox/s"}
 
 
 def oracle_sample(w, dn, f0, em, nref, budget_s=15.0, slices=None):
@@ -373,6 +403,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-probe", action="store_true")
+    ap.add_argument("--no-batch", action="store_true", help="skip the C5 batched-fields timing")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     args = ap.parse_args()

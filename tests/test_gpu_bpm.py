@@ -89,12 +89,12 @@ def test_oversampled_grids_skip_the_evanescent_band(oracle_mod, Nx, Ny, dx, nlo,
     assert np.isfinite(I).all() and np.isfinite(u).all()
 
 
+@pytest.mark.parametrize("N,B", [(128, 3), (256, 5), (512, 2)])       # 32-point-thread and 16-point-thread kernels
 @pytest.mark.parametrize("flags", ["per_field", "accumulate", "per_field+accumulate", "per_phase"])
-def test_flags(oracle_mod, flags):
+def test_flags(oracle_mod, flags, N, B):
     bb = need_gpu()
-    w = wl.tiny(N=128, Nz=6, n_cells=10, r_lo=0.5, r_hi=3.0)
+    w = wl.tiny(N=N, Nz=6, n_cells=10, r_lo=0.5, r_hi=3.0)
     dn = wl.make_dn(w)
-    B = 3
     f0 = wl.random_field(w.Nx, w.Ny, seed=11, batch=B)
     fl = 0
     if "per_field" in flags:
@@ -112,9 +112,10 @@ def test_flags(oracle_mod, flags):
     assert rel_l2(I, Io) < 2 * small_tol(w.Nz)
 
 
-def test_per_phase_launches_equal_the_persistent_kernel_bitwise():
+@pytest.mark.parametrize("cfg", ["C1", "C2"])                         # 32-point-thread / 16-point-thread kernel
+def test_per_phase_launches_equal_the_persistent_kernel_bitwise(cfg):
     bb = need_gpu()
-    w = wl.config("C1").with_nz(24)
+    w = wl.config(cfg).with_nz(24)
     dn = wl.make_dn(w).cuda()
     f0 = torch.from_numpy(wl.make_field(w)).cuda()
     out = []
