@@ -218,7 +218,7 @@ def run_ours(args):
     hbm_b, l2_b, flop = algorithmic_per_step(w)
     hbm_peak, hbm_src = measured_peaks()
     dur = prop_ms * 1e-3
-    traffic = committed_dram_traffic(w.name if not args.nz else "")
+    traffic = committed_dram_traffic(w.name if (not args.nz and B == 1) else "")
     alu_ach = flop * w.Nz / dur / 1e12
     result["roofline"] = {"bound": "alu", "achieved": alu_ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
                           "frac": alu_ach / FP32_PEAK_TFLOPS, "traffic": traffic,
