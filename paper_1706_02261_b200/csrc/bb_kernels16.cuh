@@ -152,6 +152,14 @@ __device__ __forceinline__ unsigned live_mask16(int F, int N, int c, int e0, int
     return (((1u << nl) - 1u) | ~((1u << nh) - 1u)) & 0xFFFFu;
 }
 
+// What a thread derives from the live band F of a phase (unit range of the CTA, first unit of the
+// team, load mask): recomputed only when F changes, i.e. when the reference index does -- every
+// instruction of a phase prologue is paid by all 16 warps with nothing to overlap it.
+struct UnitCache {
+    int F = -1, a0 = 0, a1 = 0, u0 = 0;
+    unsigned lmask = 0xFFFFu;
+};
+
 struct HalfWarpSync {
     unsigned mask;
     __device__ __forceinline__ void operator()() const { __syncwarp(mask); }
@@ -271,7 +279,7 @@ __device__ __forceinline__ void stage_rows_screen(const KParams &K, const Phase1
 // ----------------------------------------------------------------------------------------
 template <int P, int CW, bool ROW, int NX, int NY, bool BATCH>
 __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, const cf *sm_tw, const cf *sm_twc,
-                                            cf *sm_y, cf *sm_pw, PwTag &tag, int Fin, int Fout, int cwc) {
+                                            cf *sm_y, cf *sm_pw, PwTag &tag, UnitCache &uc, int Fin, int Fout, int cwc) {
     typedef Team16<P, CW> TM;
     constexpr int S1 = ROW ? +1 : -1, S2 = -S1;
     constexpr int JP = TM::JP;
@@ -281,17 +289,21 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
     const TM tm;
     // rows: all of them; columns: the live tiles of this step (Fin), spread evenly over the CTAs
     constexpr int CWL = CW == 8 ? 3 : (CW == 4 ? 2 : 0);
-    const LiveCols<ROW ? 1 : (NX / kL)> lv(Fin, NX, CWL);
-    const int NU = ROW ? NY : lv.total();
-    const int a0 = (int)(((long long)NU * blockIdx.x) / gridDim.x);
-    const int a1 = (int)(((long long)NU * (blockIdx.x + 1)) / gridDim.x);
-    // row phase: which of the thread's 16 sub-line elements sit in live column tiles on input (what
-    // the previous column phase wrote; the rest is stale and stands for zeros)
-    unsigned lmask = 0xFFFFu;
-    if constexpr (ROW) {
-        const int cwl = cwc == 4 ? 2 : 3;
-        lmask = live_mask16<P>(Fin, NX, tm.c, tm.t, cwl);
+    typedef LiveCols<ROW ? 1 : (NX / kL)> LV;
+    if (uc.F != Fin) {
+        const LV lv(Fin, NX, CWL);
+        const int NU0 = ROW ? NY : lv.total();
+        uc.a0 = (int)((unsigned)NU0 * blockIdx.x / gridDim.x);              // NU <= 1024: fits 32 bits
+        uc.a1 = (int)((unsigned)NU0 * (blockIdx.x + 1) / gridDim.x);
+        uc.u0 = ROW ? uc.a0 + tm.team : lv.tile(uc.a0 + tm.team);
+        // row phase: which of the thread's 16 sub-line elements sit in live column tiles on input
+        // (what the previous column phase wrote; the rest is stale and stands for zeros)
+        if constexpr (ROW) uc.lmask = live_mask16<P>(Fin, NX, tm.c, tm.t, cwc == 4 ? 2 : 3);
+        uc.F = Fin;
     }
+    const int a0 = uc.a0, a1 = uc.a1;
+    const unsigned lmask = uc.lmask;
+    const int NU = ROW ? NY : (BATCH ? LV(Fin, NX, CWL).total() : 0);
     (void)Fout;
     cf *ybuf = sm_y + ((threadIdx.x / (16 * CW)) * (16 * 17 * CW)) + tm.col;        // one region per (team, class)
     cf *xbuf = sm_y + tm.team * (TM::TEAM * 17) + tm.col;                            // same memory, team's part
@@ -327,7 +339,7 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
     const int k1 = BATCH ? (ROW ? a1 * B : (int)(((long long)NU * B * (blockIdx.x + 1)) / gridDim.x)) : a1;
     for (int k = k0 + tm.team; k < k1; k += TM::NTEAM) {
         const int m = BATCH ? k / B : k, b = BATCH ? k - m * B : 0;
-        const int u = ROW ? m : lv.tile(m);
+        const int u = ROW ? m : (!BATCH && k == k0 + tm.team ? uc.u0 : LV(Fin, NX, CWL).tile(m));
         if constexpr (BATCH && ROW) {
             pw = sm_pw + (m - a0) * NX;                         // the row's factors, indexed by pixel
         } else if (d.kind != 0 && (tag.src != d.src || tag.pix0 != u)) {
@@ -402,7 +414,7 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
                         float I = fmaf(w.x, w.x, w.y * w.y);
                         float *a = ip + tm.q(jp) + kL * mm;
                         if (accumulate) I += *a;
-                        __stcs(a, I);
+                        __stcg(a, I);
                     }
             }
         } else if (d.kind == 2) {
@@ -509,6 +521,7 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const KParams P) {
     __syncthreads();
 
     PwTag tagH = {nullptr, -1}, tagS = {nullptr, -1};
+    UnitCache ucR, ucC;
     // largest live |kx bin| of the step whose column phase wrote (Fa) / will read (Fb) the field of a
     // phase; fetched one phase ahead so that the global load is not on the critical path
     auto live_in = [&](int p) {
@@ -520,6 +533,7 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const KParams P) {
         return row ? ((p >> 1) < P.Nz_total ? P.fmax[p >> 1] : NX / 2) : P.fmax[p >> 1];
     };
     int Fa_next = live_in(P.p0), Fb_next = live_out(P.p0);
+    Phase16 d_next = decode_phase16(P, P.p0);
     unsigned nbar = 0;
     // optional timeline (bb_probe_trace): per phase and CTA, clock64 at phase start / work done /
     // arrived / prefilled / released, and the global timer at release
@@ -527,7 +541,7 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const KParams P) {
     const bool tracer = tr != nullptr && threadIdx.x == 0;
 #pragma unroll 1
     for (int p = P.p0; p < P.p1; ++p) {
-        const Phase16 d = decode_phase16(P, p);
+        const Phase16 d = d_next;              // decoded while the previous barrier was pending
         if (tracer) tr[0] = clock64();
         if (d.is_row && p + 2 < P.p1) {
             // the dn rows this CTA turns into screen factors at the end of this phase (for the row
@@ -542,8 +556,8 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const KParams P) {
         }
         // largest live |kx bin| of the step whose column phase wrote / will read the field
         const int Fa = Fa_next, Fb = Fb_next;
-        if (d.is_row) run_phase16<PX, 1, true, NX, NY, BATCH>(P, d, sm_tw, sm_twcx, sm_y, sm_pwS, tagS, Fa, Fb, CWC);
-        else run_phase16<PY, CWC, false, NX, NY, BATCH>(P, d, sm_tw, sm_twcy, sm_y, sm_pwH, tagH, Fa, Fa, CWC);
+        if (d.is_row) run_phase16<PX, 1, true, NX, NY, BATCH>(P, d, sm_tw, sm_twcx, sm_y, sm_pwS, tagS, ucR, Fa, Fb, CWC);
+        else run_phase16<PY, CWC, false, NX, NY, BATCH>(P, d, sm_tw, sm_twcy, sm_y, sm_pwH, tagH, ucC, Fa, Fa, CWC);
         if (tracer) tr[1] = clock64();
         if (BATCH && d.is_row && d.kind == 1 && P.inten != nullptr && !(P.flags & 2u) && P.B > 1)
             tagH.src = nullptr;                // the intensity sums used the propagator buffer
@@ -553,17 +567,18 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const KParams P) {
             if (tracer) tr[2] = clock64();
             Fa_next = live_in(p + 1);
             Fb_next = live_out(p + 1);
+            d_next = decode_phase16(P, p + 1);   // its global loads (table pointer, phase offset) overlap the barrier
             // While the barrier is pending, stage what does not depend on the field.  After a row
             // phase: the propagator values of the coming column phase (only when the table changed)
             // and the screen factors of the NEXT row phase (its dn slice is known), so that the
             // sin/cos work has a whole barrier + column phase of slack.  After a column phase:
             // the screen factors, if they are not there yet (first row phase of a launch).
             if (d.is_row) {
-                const int Fn = P.fmax[(p + 1) >> 1];
-                prefill_phase16<PY, CWC, false, NX, NY, BATCH>(P, decode_phase16(P, p + 1), sm_pwH, tagH, Fn);
+                const int Fn = Fa_next;
+                prefill_phase16<PY, CWC, false, NX, NY, BATCH>(P, d_next, sm_pwH, tagH, Fn);
                 if (p + 2 < P.p1) prefill_phase16<PX, 1, true, NX, NY, BATCH>(P, decode_phase16(P, p + 2), sm_pwS, tagS, 0);
             } else {
-                prefill_phase16<PX, 1, true, NX, NY, BATCH>(P, decode_phase16(P, p + 1), sm_pwS, tagS, 0);
+                prefill_phase16<PX, 1, true, NX, NY, BATCH>(P, d_next, sm_pwS, tagS, 0);
             }
             if (tracer) tr[3] = clock64();
             if (grid_wait(P.bar, nbar * gridDim.x, P.status, sm_abort)) return;
