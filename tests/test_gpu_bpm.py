@@ -127,6 +127,30 @@ def test_per_phase_launches_equal_the_persistent_kernel_bitwise(cfg):
     assert torch.equal(out[0][0], out[1][0]) and torch.equal(out[0][1], out[1][1])
 
 
+@pytest.mark.parametrize("Nx,Ny,dx", [(1024, 1024, 0.1), (512, 1024, 0.2), (256, 256, 0.08)])
+def test_repeated_runs_are_bit_identical(Nx, Ny, dx):
+    """compute-sanitizer is closed on this pool, so shared-memory hazards of the 16-point-thread
+    kernel (exchange buffer aliased on the transposes, named barriers per team) are looked for the
+    other way round: a race would make repeated runs differ.  Single field: no atomics, so the
+    result is deterministic by construction."""
+    bb = need_gpu()
+    w = wl.tiny(N=Nx, Nz=12, n_cells=10, r_lo=0.5, r_hi=3.0)
+    w = wl.dataclasses.replace(w, Ny=Ny, dx=dx)
+    dn = wl.make_dn(w).cuda()
+    f0 = torch.from_numpy(wl.random_field(Nx, Ny, seed=5, batch=1)).cuda()
+    nref = np.linspace(1.30, 1.40, w.Nz).astype(np.float32)
+    ref = None
+    for rep in range(4):
+        d, I = f0.clone(), torch.full(dn.shape, float("nan"), device="cuda")
+        bb.propagate(d, dn, w.dx, w.dz, w.lam, w.n0, intensity=I, nref=nref)
+        torch.cuda.synchronize()
+        if ref is None:
+            ref = (d, I)
+        else:
+            assert torch.equal(d, ref[0]) and torch.equal(I, ref[1])
+    bb.device_status()
+
+
 def test_flat_entry_point_null_intensity_and_nref_variants(oracle_mod):
     bb = need_gpu()
     w = wl.config("C1").with_nz(16)
