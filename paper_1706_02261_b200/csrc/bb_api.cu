@@ -764,13 +764,29 @@ int bb_multiplex_psf(const float *pos, const float *phase, const float *amp, int
         for (int i = 0; i < Nx; ++i)
             if (kx2[i] + ky2[q] <= kc2) ++count;
     if (count == 0) return fail(BB_ERR_INVALID_ARG, "pupil of NA = %g contains no grid frequency", (double)NA);
-    rc = ws_reserve(g_ws_misc, std::max<size_t>((size_t)M * sizeof(bb::EmitterPrep), 4096));
+    // bounding box of the pupil in DFT bins: [-F, F] per axis, clipped to [-N/2, N/2 - 1]
+    auto extent = [&](const std::vector<double> &k2, int N, int *lo, int *w) {
+        int F = 0;
+        for (int f = 0; f <= N / 2; ++f)
+            if (k2[f] <= kc2) F = f;
+        *lo = std::min(F, N / 2);
+        *w = *lo + std::min(F, N / 2 - 1) + 1;
+    };
+    int Fx, Wx, Fy, Wy;
+    extent(kx2, Nx, &Fx, &Wx);
+    extent(ky2, Ny, &Fy, &Wy);
+    const size_t em_bytes = (((size_t)M * sizeof(bb::EmitterPrep)) + 255) & ~(size_t)255;
+    rc = ws_reserve(g_ws_misc, em_bytes + (size_t)M * (Wx + Wy) * sizeof(cf) + 4096);
     if (rc) return rc;
     bb::EmitterPrep *em = (bb::EmitterPrep *)g_ws_misc.ptr;
+    cf *EX = (cf *)((char *)g_ws_misc.ptr + em_bytes), *EY = EX + (size_t)M * Wx;
     bb::emitter_prep_kernel<<<(M + 127) / 128, 128, 0, s>>>(pos, phase, amp, M, Nx, Ny, ddx, em);
     ++g_launches;
-    dim3 block(128), grid((Nx + 127) / 128, Ny);
-    bb::multiplex_spectrum_kernel<<<grid, block, 128 * sizeof(bb::EmitterPrep), s>>>((cf *)field_out, Nx, Ny, ddx, kc2, em, M);
+    bb::emitter_axis_kernel<<<dim3((std::max(Wx, Wy) + 127) / 128, M), 128, 0, s>>>(em, M, Fx, Wx, Fy, Wy, EX, EY);
+    ++g_launches;
+    BB_CUDA(cudaMemsetAsync(field_out, 0, (size_t)Nx * Ny * sizeof(cf), s));
+    bb::multiplex_gemm_kernel<<<dim3((Wx + 31) / 32, (Wy + 31) / 32), 256, 0, s>>>((cf *)field_out, Nx, Ny, ddx, kc2, EX, EY,
+                                                                                   M, Fx, Wx, Fy, Wy);
     ++g_launches;
     BB_CUDA(cudaGetLastError());
     bb::PhaseProg prog[2];

@@ -53,39 +53,77 @@ __global__ void emitter_prep_kernel(const float *__restrict__ pos, const float *
 }
 
 // U0[q][p] = P * sum_e a_e exp(i (phi_e - kx X_e - ky Y_e))   (bb.h bb_multiplex_psf; readings A12-A14).
-// kx X_e = 2 pi f_p (X_e / (Nx dx)): the product f_p * ax is reduced mod 1 in double, the
-// remaining angle (|.| <= pi + |phi|) goes through single-precision sincos.
-__global__ void multiplex_spectrum_kernel(float2 *__restrict__ U0, int Nx, int Ny, double dx, double kc2,
-                                          const EmitterPrep *__restrict__ em, int M) {
+// kx X_e = 2 pi f_p (X_e / (Nx dx)): the product f_p * ax is reduced mod 1 in double, the remaining
+// angle (|.| <= pi + |phi|) goes through single-precision sincos.  Separable form:
+// the phase ramp factorises,
+//   a_e exp(i (phi_e - kx X_e - ky Y_e)) = [a_e exp(i (phi_e - kx X_e))] [exp(-i ky Y_e)] = EX[e][p] EY[e][q],
+// so the sum over emitters is a complex matrix product over the bounding box of the pupil,
+//   U0[q][p] = P[q][p] sum_e EY[e][q] EX[e][p]      (M x Wy)^T (M x Wx),
+// instead of one sincos per (pixel, emitter).
+// Bins f = i - Fx (i < Wx) along x, f = i - Fy (i < Wy) along y: [-F, F] clipped to [-N/2, N/2 - 1].
+__global__ void emitter_axis_kernel(const EmitterPrep *__restrict__ em, int M, int Fx, int Wx, int Fy, int Wy,
+                                    float2 *__restrict__ EX, float2 *__restrict__ EY) {
+    const int e = blockIdx.y;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= M) return;
+    const EmitterPrep E = em[e];
+    if (i < Wx) {
+        const double tt = (double)(i - Fx) * E.ax;
+        const float r = (float)(tt - rint(tt));
+        float s, c;
+        sincosf(fmaf(-6.283185307179586f, r, E.phase), &s, &c);
+        EX[(size_t)e * Wx + i] = make_float2(E.amp * c, E.amp * s);
+    }
+    if (i < Wy) {
+        const double tt = (double)(i - Fy) * E.ay;
+        const float r = (float)(tt - rint(tt));
+        float s, c;
+        sincosf(-6.283185307179586f * r, &s, &c);
+        EY[(size_t)e * Wy + i] = make_float2(c, s);
+    }
+}
+
+// U0 over the pupil's bounding box: 32 x 32 outputs per CTA (256 threads, 2 x 2 each), emitters in
+// chunks of 32 through shared memory.  U0 must have been zeroed (pixels outside the box stay zero).
+__global__ void __launch_bounds__(256) multiplex_gemm_kernel(float2 *__restrict__ U0, int Nx, int Ny, double dx, double kc2,
+                                                             const float2 *__restrict__ EX, const float2 *__restrict__ EY,
+                                                             int M, int Fx, int Wx, int Fy, int Wy) {
     const double two_pi = 6.283185307179586476925286766559;
-    extern __shared__ EmitterPrep sm_em[];
-    int p = blockIdx.x * blockDim.x + threadIdx.x;
-    int q = blockIdx.y;
-    int fp = freq_index(p < Nx ? p : 0, Nx), fq = freq_index(q, Ny);
-    double kx = __ddiv_rn(__dmul_rn(two_pi, (double)fp), __dmul_rn((double)Nx, dx));
-    double ky = __ddiv_rn(__dmul_rn(two_pi, (double)fq), __dmul_rn((double)Ny, dx));
-    bool inside = (p < Nx) && (__dadd_rn(__dmul_rn(kx, kx), __dmul_rn(ky, ky)) <= kc2);
-    float sr = 0.f, si = 0.f;
-    // whole blocks outside the pupil skip the emitter loop
-    if (__syncthreads_or(inside ? 1 : 0)) {
-        for (int e0 = 0; e0 < M; e0 += blockDim.x) {
-            int n = min((int)blockDim.x, M - e0);
-            __syncthreads();
-            if ((int)threadIdx.x < n) sm_em[threadIdx.x] = em[e0 + threadIdx.x];
-            __syncthreads();
-            if (inside) {
-                for (int e = 0; e < n; ++e) {
-                    double tt = (double)fp * sm_em[e].ax + (double)fq * sm_em[e].ay;
-                    float r = (float)(tt - rint(tt));
-                    float s, c;
-                    sincosf(fmaf(-6.283185307179586f, r, sm_em[e].phase), &s, &c);
-                    sr = fmaf(sm_em[e].amp, c, sr);
-                    si = fmaf(sm_em[e].amp, s, si);
-                }
-            }
+    constexpr int TK = 32;
+    __shared__ float2 sx[TK][32], sy[TK][32];
+    const int tx = threadIdx.x % 16, ty = threadIdx.x / 16;           // outputs (ty + 16 a, tx + 16 b), a, b < 2
+    const int i0 = blockIdx.x * 32, j0 = blockIdx.y * 32;
+    float2 acc[2][2] = {};
+    for (int e0 = 0; e0 < M; e0 += TK) {
+        __syncthreads();
+        for (int l = threadIdx.x; l < TK * 32; l += 256) {
+            const int k = l / 32, c = l % 32, e = e0 + k;
+            sx[k][c] = (e < M && i0 + c < Wx) ? EX[(size_t)e * Wx + i0 + c] : make_float2(0.f, 0.f);
+            sy[k][c] = (e < M && j0 + c < Wy) ? EY[(size_t)e * Wy + j0 + c] : make_float2(0.f, 0.f);
+        }
+        __syncthreads();
+#pragma unroll 8
+        for (int k = 0; k < TK; ++k) {
+            const float2 x0 = sx[k][tx], x1 = sx[k][tx + 16], y0 = sy[k][ty], y1 = sy[k][ty + 16];
+            acc[0][0].x = fmaf(y0.x, x0.x, fmaf(-y0.y, x0.y, acc[0][0].x)); acc[0][0].y = fmaf(y0.x, x0.y, fmaf(y0.y, x0.x, acc[0][0].y));
+            acc[0][1].x = fmaf(y0.x, x1.x, fmaf(-y0.y, x1.y, acc[0][1].x)); acc[0][1].y = fmaf(y0.x, x1.y, fmaf(y0.y, x1.x, acc[0][1].y));
+            acc[1][0].x = fmaf(y1.x, x0.x, fmaf(-y1.y, x0.y, acc[1][0].x)); acc[1][0].y = fmaf(y1.x, x0.y, fmaf(y1.y, x0.x, acc[1][0].y));
+            acc[1][1].x = fmaf(y1.x, x1.x, fmaf(-y1.y, x1.y, acc[1][1].x)); acc[1][1].y = fmaf(y1.x, x1.y, fmaf(y1.y, x1.x, acc[1][1].y));
         }
     }
-    if (p < Nx) U0[(size_t)q * Nx + p] = inside ? make_float2(sr, si) : make_float2(0.f, 0.f);
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+        for (int b = 0; b < 2; ++b) {
+            const int j = j0 + ty + 16 * a, i = i0 + tx + 16 * b;
+            if (j >= Wy || i >= Wx) continue;
+            const int fq = j - Fy, fp = i - Fx;
+            const double kx = __ddiv_rn(__dmul_rn(two_pi, (double)fp), __dmul_rn((double)Nx, dx));
+            const double ky = __ddiv_rn(__dmul_rn(two_pi, (double)fq), __dmul_rn((double)Ny, dx));
+            if (!(__dadd_rn(__dmul_rn(kx, kx), __dmul_rn(ky, ky)) <= kc2)) continue;
+            const int p = fp >= 0 ? fp : fp + Nx, q = fq >= 0 ? fq : fq + Ny;
+            U0[(size_t)q * Nx + p] = acc[a][b];
+        }
 }
 
 // Per-slice partial sums of dn in double: partial[j][blockIdx.x] (fixed summation order,
