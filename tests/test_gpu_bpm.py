@@ -151,9 +151,10 @@ def test_repeated_runs_are_bit_identical(Nx, Ny, dx):
     bb.device_status()
 
 
-def test_flat_entry_point_null_intensity_and_nref_variants(oracle_mod):
+@pytest.mark.parametrize("cfg", ["C1", "C2"])                         # 32-point-thread / 16-point-thread kernel
+def test_flat_entry_point_null_intensity_and_nref_variants(oracle_mod, cfg):
     bb = need_gpu()
-    w = wl.config("C1").with_nz(16)
+    w = wl.config(cfg).with_nz(16)
     dn = wl.make_dn(w)
     f0 = wl.make_field(w)
     uo, Io = oracle_mod.propagate(f0[0], dn.numpy(), w.dx, w.dz, w.lam, w.n0)
@@ -189,6 +190,27 @@ def test_more_reference_indices_than_cached_tables(oracle_mod, monkeypatch):
         monkeypatch.delenv("BB_TABLE_CACHE_MB")
         bb.shutdown()
     assert rel_l2(u, uo) < small_tol(7) and rel_l2(I, Io) < 2 * small_tol(7)
+
+
+def test_host_buffer_entry_point_with_a_batch(oracle_mod):
+    """Host buffers, B = 3 fields on a 256 x 512 grid (batch variant of the 16-point-thread kernel),
+    dn streamed in several chunks; summed intensity (shared-memory atomics: compared to tolerance)."""
+    bb = need_gpu()
+    w = wl.tiny(N=256, Nz=70, n_cells=12, r_lo=0.5, r_hi=3.0)
+    w = wl.dataclasses.replace(w, Ny=512)
+    dn = wl.make_dn(w)
+    f0 = wl.random_field(w.Nx, w.Ny, seed=9, batch=3)
+    nref = oracle_mod.nref_from_dn(dn.numpy(), w.n0, 16)
+    d = torch.from_numpy(f0.copy()).cuda()
+    I = torch.empty(dn.shape, device="cuda")
+    bb.propagate(d, dn.cuda(), w.dx, w.dz, w.lam, w.n0, intensity=I, nref=nref)
+    fh = torch.from_numpy(f0.copy()).pin_memory()
+    Ih = torch.empty(dn.shape).pin_memory()
+    bb.propagate(fh, dn.pin_memory(), w.dx, w.dz, w.lam, w.n0, intensity=Ih, nref=nref)
+    assert torch.equal(fh, d.cpu())
+    assert rel_l2(Ih.numpy(), I.cpu().numpy().astype(np.float64)) < 1e-6
+    uo, Io = oracle_mod.propagate(f0[1], dn.numpy(), w.dx, w.dz, w.lam, w.n0, nref=nref)
+    assert rel_l2(fh.numpy()[1], uo) < small_tol(w.Nz)
 
 
 def test_host_buffer_entry_point_equals_device_entry_point(oracle_mod):
