@@ -259,8 +259,8 @@ __device__ __forceinline__ void fill_pw16(int kind, const void *src, int unit, f
 // apply them to the B fields.
 template <int NX, int NY>
 __device__ __forceinline__ void stage_rows_screen(const KParams &K, const Phase16 &d, cf *pw) {
-    const int a0 = (int)(((long long)NY * blockIdx.x) / gridDim.x);
-    const int a1 = (int)(((long long)NY * (blockIdx.x + 1)) / gridDim.x);
+    const int a0 = (int)((unsigned)NY * blockIdx.x / gridDim.x);
+    const int a1 = (int)((unsigned)NY * (blockIdx.x + 1) / gridDim.x);
     const int total = (a1 - a0) * NX;
     const float *dnp = reinterpret_cast<const float *>(d.src) + (long long)a0 * NX;
 #pragma unroll 4
@@ -486,8 +486,8 @@ __device__ __forceinline__ void prefill_phase16(const KParams &K, const Phase16 
     const TM tm;
     const LiveCols<ROW ? 1 : (NX / kL)> lv(Fin, NX, CW == 8 ? 3 : (CW == 4 ? 2 : 0));
     const int NU = ROW ? NY : lv.total();
-    const int a0 = (int)(((long long)NU * blockIdx.x) / gridDim.x);
-    const int a1 = (int)(((long long)NU * (blockIdx.x + 1)) / gridDim.x);
+    const int a0 = (int)((unsigned)NU * blockIdx.x / gridDim.x);              // NU <= 1024: fits 32 bits
+    const int a1 = (int)((unsigned)NU * (blockIdx.x + 1) / gridDim.x);
     const int B = BATCH ? K.B : 1;
     const int k0 = BATCH ? (int)(((long long)NU * B * blockIdx.x) / gridDim.x) : a0;
     const int k1 = BATCH ? (int)(((long long)NU * B * (blockIdx.x + 1)) / gridDim.x) : a1;
@@ -534,6 +534,8 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const KParams P) {
     };
     int Fa_next = live_in(P.p0), Fb_next = live_out(P.p0);
     Phase16 d_next = decode_phase16(P, P.p0);
+    const int r0 = (int)((unsigned)NY * blockIdx.x / gridDim.x);          // rows of this CTA (row phases)
+    const int r1 = (int)((unsigned)NY * (blockIdx.x + 1) / gridDim.x);
     unsigned nbar = 0;
     // optional timeline (bb_probe_trace): per phase and CTA, clock64 at phase start / work done /
     // arrived / prefilled / released, and the global timer at release
@@ -546,8 +548,6 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const KParams P) {
         if (d.is_row && p + 2 < P.p1) {
             // the dn rows this CTA turns into screen factors at the end of this phase (for the row
             // phase after next): start them on their way from HBM to L2 now, one bulk prefetch per row
-            const int r0 = (int)(((long long)NY * blockIdx.x) / gridDim.x);
-            const int r1 = (int)(((long long)NY * (blockIdx.x + 1)) / gridDim.x);
             if ((int)threadIdx.x < r1 - r0) {
                 const float *row = P.dn + (long long)((p >> 1) - P.j_base) * ((long long)NX * NY)
                                    + (long long)(r0 + threadIdx.x) * NX;
