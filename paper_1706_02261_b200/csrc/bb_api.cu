@@ -327,7 +327,7 @@ int launch_steps(Plan *p, cf *field, const float *dn, float *inten, long long in
     P.mode = 0;
     P.twx = p->twx; P.twy = p->twy; P.bar = p->bar; P.status = p->status;
     P.tw256 = p->tw256; P.twcx = p->twcx; P.twcy = p->twcy;
-    P.fmax = p->d_fmax; P.cw4 = p->cw4; P.zeros = (const cf *)(p->status + 16);
+    P.fmax = p->d_fmax; P.cw4 = p->cw4;
     P.flags = flags & 3u;
     const bool k16 = use_k16(p, B);
     if (g_trace && k16 && 2 * j1 + 1 <= g_trace_phases) { P.trace = g_trace; P.trace_p0 = 0; }

@@ -52,7 +52,6 @@ struct KParams {
     int *status;               // device flag: != 0 -> watchdog tripped
     unsigned flags;            // BB_ACCUMULATE = 1, BB_INTENSITY_PER_FIELD = 2
     const int *fmax;           // device [Nz_total]: largest |kx DFT bin| the propagator of step j lets through (conservative)
-    const cf *zeros;           // a few zero elements in global memory
     int cw4;                   // 16-point-thread kernel: column tiles of 4 columns instead of 8
     long long *trace;          // bb_probe_trace: [phase - trace_p0][CTA][6] time stamps, or nullptr
     int trace_p0;
