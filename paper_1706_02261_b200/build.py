@@ -7,6 +7,7 @@ are compiled in parallel and linked into one shared library next to this file.
 from __future__ import annotations
 
 import concurrent.futures
+import hashlib
 import os
 import subprocess
 import sys
@@ -33,6 +34,18 @@ def _sources():
     return deps
 
 
+def _digest(deps) -> str:
+    """Content hash of the sources: a copy of the tree (fresh mtimes, e.g. on the GPU box) must not
+    trigger a rebuild of an up-to-date library."""
+    h = hashlib.sha256()
+    for d in deps:
+        h.update(os.path.basename(d).encode())
+        with open(d, "rb") as f:
+            h.update(f.read())
+    h.update(" ".join(NVCC_FLAGS[:-1]).encode())
+    return h.hexdigest()
+
+
 def _stale(target: str, deps) -> bool:
     if not os.path.exists(target):
         return True
@@ -49,8 +62,12 @@ def _run(cmd):
 
 def build_library(force: bool = False, verbose: bool = False) -> str:
     deps = _sources()
-    if not force and not _stale(LIB, deps):
-        return LIB
+    stamp = LIB + ".sha256"
+    digest = _digest(deps)
+    if not force and os.path.exists(LIB) and os.path.exists(stamp):
+        with open(stamp) as f:
+            if f.read().strip() == digest:
+                return LIB
     os.makedirs(OBJ, exist_ok=True)
     nvcc = _nvcc()
     jobs = []
@@ -67,7 +84,7 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
     jobs.append((obj_api, [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, "bb_api.cu"), "-o", obj_api]))
     obj_probe = os.path.join(OBJ, "bb_probe.o")
     jobs.append((obj_probe, [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, "bb_probe.cu"), "-o", obj_probe]))
-    todo = [(o, c) for o, c in jobs if force or _stale(o, deps)]
+    todo = [(o, c) for o, c in jobs if force or _stale(o, deps)]          # objects newer than every source are kept
     with concurrent.futures.ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
         for out in ex.map(lambda oc: _run(oc[1]), todo):
             if verbose and out.strip():
@@ -76,6 +93,8 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
     _run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp, *[o for o, _ in jobs],
           "-lcudart_static", "-ldl", "-lrt", "-lpthread"])
     os.replace(tmp, LIB)
+    with open(stamp, "w") as f:
+        f.write(digest + "\n")
     return LIB
 
 
