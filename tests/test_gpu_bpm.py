@@ -290,6 +290,15 @@ def test_config_c5_batched_parity(oracle_mod):
 
 
 @pytest.mark.slow
+def test_config_c5_batched_parity_full(oracle_mod):
+    """configs[4] at full size (16 fields of 512^2 through all 512 slices, summed intensity): every
+    element of the 16 final fields and of the intensity volume (the oracle runs 16 propagations)."""
+    bb = need_gpu()
+    err_u, err_I = _full_config_parity(bb, oracle_mod, "C5")
+    assert err_u < TOL and err_I < TOL
+
+
+@pytest.mark.slow
 def test_config_c4_headline_parity_full(oracle_mod):
     """configs[3], the workload bench.py times, at full size (1024^2 x 1024 steps) in the same
     launch configuration: every element of the final field and of the 4 GiB intensity volume."""
