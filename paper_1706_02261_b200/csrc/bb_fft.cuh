@@ -18,8 +18,20 @@ namespace bb {
 
 typedef float2 cf;
 
-__device__ __forceinline__ cf cadd(cf a, cf b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ cf csub(cf a, cf b) { return make_float2(a.x - b.x, a.y - b.y); }
+// Complex add / subtract as ONE packed instruction (FADD2, sm_100): same lane throughput as two FADDs
+// but half the issue slots, and the butterflies are two thirds additions.  Same rounding (rn per lane).
+__device__ __forceinline__ cf cadd(cf a, cf b) {
+    unsigned long long r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r)
+        : "l"(*reinterpret_cast<unsigned long long *>(&a)), "l"(*reinterpret_cast<unsigned long long *>(&b)));
+    return *reinterpret_cast<cf *>(&r);
+}
+__device__ __forceinline__ cf csub(cf a, cf b) {
+    unsigned long long r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r)
+        : "l"(*reinterpret_cast<unsigned long long *>(&a)), "l"(*reinterpret_cast<unsigned long long *>(&b)));
+    return *reinterpret_cast<cf *>(&r);
+}
 // a * w
 __device__ __forceinline__ cf cmul(cf a, cf w) {
     return make_float2(fmaf(a.x, w.x, -(a.y * w.y)), fmaf(a.x, w.y, a.y * w.x));
