@@ -32,6 +32,20 @@ __device__ __forceinline__ cf csub(cf a, cf b) {
         : "l"(*reinterpret_cast<unsigned long long *>(&a)), "l"(*reinterpret_cast<unsigned long long *>(&b)));
     return *reinterpret_cast<cf *>(&r);
 }
+// Packed-pair plumbing: ptxas folds the pair construction into operand selectors (scalar broadcast
+// R.F32, swapped halves R.F32x2.LO_HI), so these cost no instructions.
+typedef unsigned long long u64;
+__device__ __forceinline__ u64 pk2(float lo, float hi) { u64 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ cf up2(u64 v) { cf r; asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v)); return r; }
+// (A, B) * (rh + rl) per lane, one rounding of t*rh + t*rl each: two packed instructions
+__device__ __forceinline__ cf mul_hilo2(float A, float B, float rh, float rl) {
+    u64 t, r;
+    const u64 ab = pk2(A, B);
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(t) : "l"(ab), "l"(pk2(rl, rl)));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(ab), "l"(pk2(rh, rh)), "l"(t));
+    return up2(r);
+}
+
 // a * w
 __device__ __forceinline__ cf cmul(cf a, cf w) {
     return make_float2(fmaf(a.x, w.x, -(a.y * w.y)), fmaf(a.x, w.y, a.y * w.x));
@@ -89,11 +103,9 @@ __device__ __forceinline__ cf mul_w32(cf a) {
         constexpr float rh = hi_of(cos32d(4)), rl = lo_of(cos32d(4));
         const float p = a.x + a.y, q = a.y - a.x;       // p = x + y, q = y - x
         if constexpr (M == 4)
-            return SIGN < 0 ? make_float2(mul_hilo(p, rh, rl), mul_hilo(q, rh, rl))
-                            : make_float2(mul_hilo(-q, rh, rl), mul_hilo(p, rh, rl));
+            return SIGN < 0 ? mul_hilo2(p, q, rh, rl) : mul_hilo2(-q, p, rh, rl);
         else
-            return SIGN < 0 ? make_float2(mul_hilo(q, rh, rl), mul_hilo(-p, rh, rl))
-                            : make_float2(mul_hilo(-p, rh, rl), mul_hilo(-q, rh, rl));
+            return SIGN < 0 ? mul_hilo2(q, -p, rh, rl) : mul_hilo2(-p, -q, rh, rl);
     } else {
         constexpr double cd = cos32d(M), sd = SIGN < 0 ? -sin32d(M) : sin32d(M);
         constexpr float c = hi_of(cd), cl = lo_of(cd), s = hi_of(sd), sl = lo_of(sd);
