@@ -16,6 +16,7 @@
 // screen or propagator values) are staged in a thread-private shared-memory column
 // -- filled while the grid barrier before the phase is pending.
 #pragma once
+#include <cuda.h>
 #include "bb_fft.cuh"
 
 namespace bb {
@@ -53,8 +54,12 @@ struct KParams {
     unsigned flags;            // BB_ACCUMULATE = 1, BB_INTENSITY_PER_FIELD = 2
     const int *fmax;           // device [Nz_total]: largest |kx DFT bin| the propagator of step j lets through (conservative)
     int cw4;                   // 16-point-thread kernel: column tiles of 4 columns instead of 8
+    int use_tma;               // 16-point-thread kernel: column tiles are fetched by TMA through `tmap`
     long long *trace;          // bb_probe_trace: [phase - trace_p0][CTA][6] time stamps, or nullptr
     int trace_p0;
+    // field as a 3-D tensor (column, y mod PY, y div PY) of 8-byte elements, box = (CW, 1, 256): one
+    // TMA request brings one y-class of a column tile, [256][CW] row-major, into shared memory
+    alignas(64) CUtensorMap tmap;
 };
 
 __device__ __forceinline__ cf ld_cg(const cf *p) { return __ldcg(p); }

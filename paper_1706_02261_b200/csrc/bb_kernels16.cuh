@@ -33,7 +33,7 @@ struct Smem16 {
                                                                         // (kThreads16 * 16) reuses the same region
     static constexpr int kPw = kThreads16 * 16;                         // pointwise factors: one buffer for the
                                                                         // propagator values, one for the screen
-    static constexpr size_t bytes = (size_t)(kTw + kTwc + kY + 2 * kPw) * sizeof(cf) + 16;
+    static constexpr size_t bytes = (size_t)(kTw + kTwc + kY + 2 * kPw) * sizeof(cf) + 16 + 8 * 8;
 };
 
 struct Phase16 {
@@ -158,7 +158,31 @@ __device__ __forceinline__ unsigned live_mask16(int F, int N, int c, int e0, int
 struct UnitCache {
     int F = -1, a0 = 0, a1 = 0, u0 = 0;
     unsigned lmask = 0xFFFFu;
+    unsigned tma_parity = 0;           // phase bit of the team's TMA barrier
 };
+
+// ---- TMA / mbarrier plumbing (column tiles of the single-field kernel) ----
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+// false: gave up (a hang would take the box down; the caller raises the watchdog flag)
+__device__ __forceinline__ bool mbar_wait(unsigned long long *bar, unsigned parity) {
+    for (unsigned spins = 0; spins < (1u << 22); ++spins) {
+        unsigned ok;
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+        if (ok) return true;
+    }
+    return false;
+}
+__device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *tm, int c0, int c1, int c2, unsigned long long *bar) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+}
 
 struct HalfWarpSync {
     unsigned mask;
@@ -279,7 +303,8 @@ __device__ __forceinline__ void stage_rows_screen(const KParams &K, const Phase1
 // ----------------------------------------------------------------------------------------
 template <int P, int CW, bool ROW, int NX, int NY, bool BATCH>
 __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, const cf *sm_tw, const cf *sm_twc,
-                                            cf *sm_y, cf *sm_pw, PwTag &tag, UnitCache &uc, int Fin, int Fout, int cwc) {
+                                            cf *sm_y, cf *sm_pw, PwTag &tag, UnitCache &uc, int Fin, int Fout, int cwc,
+                                            unsigned long long *sm_mbar = nullptr) {
     typedef Team16<P, CW> TM;
     constexpr int S1 = ROW ? +1 : -1, S2 = -S1;
     constexpr int JP = TM::JP;
@@ -348,12 +373,36 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
         }
         cf *line = K.field + b * npx + (ROW ? (long long)u * NX : (long long)u * CW + tm.col);
         cf v[16];
-        if (d.first) {
-            const cf *src = line + tm.c * CS + tm.t * IS;
+        bool loaded = false;
+        if constexpr (!ROW && !BATCH) {
+            if (K.use_tma) {
+                // One thread asks the TMA unit for the P y-classes of the tile ([256][CW] each, into the
+                // team's part of the transpose region); the 16 CW strided 8 CW-byte row segments per warp
+                // load instruction, which kept the LSU busy for 0.5 us, become conflict-free LDS.
+                cf *stage = sm_y + tm.team * (TM::TEAM * 17);
+                unsigned long long *bar = sm_mbar + tm.team;
+                if (threadIdx.x % TM::TEAM == 0) {
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    mbar_expect_tx(bar, (unsigned)(P * kL * CW * sizeof(cf)));
 #pragma unroll
-            for (int i = 0; i < 16; ++i) {
-                v[i] = make_float2(0.f, 0.f);
-                if (!ROW || ((lmask >> i) & 1u)) v[i] = ld_cg(src + 16 * IS * i);
+                    for (int cc = 0; cc < P; ++cc) tma_load_3d(stage + cc * kL * CW, &K.tmap, u * CW, cc, 0, bar);
+                }
+                if (!mbar_wait(bar, uc.tma_parity)) atomicExch(K.status, 2);
+                uc.tma_parity ^= 1u;
+#pragma unroll
+                for (int i = 0; i < 16; ++i) v[i] = stage[(tm.c * kL + tm.t + 16 * i) * CW + tm.col];
+                tm.sync();                              // staged tile read: the region goes back to the transposes
+                loaded = true;
+            }
+        }
+        if (d.first) {
+            if (!loaded) {
+                const cf *src = line + tm.c * CS + tm.t * IS;
+#pragma unroll
+                for (int i = 0; i < 16; ++i) {
+                    v[i] = make_float2(0.f, 0.f);
+                    if (!ROW || ((lmask >> i) & 1u)) v[i] = ld_cg(src + 16 * IS * i);
+                }
             }
             if constexpr (ROW) subline_fft<S1, CW>(v, sm_tw, ybuf, tm.t, hsync);
             else subline_fft<S1, CW>(v, sm_tw, ybuf, tm.t, tsync);
@@ -502,8 +551,8 @@ __device__ __forceinline__ void prefill_phase16(const KParams &K, const Phase16 
 
 // CWC: columns per column tile (8, or 4 when few columns are live); BATCH: several fields (KParams::B)
 template <int PX, int PY, int CWC, bool BATCH>
-__global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const KParams P) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+__global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const __grid_constant__ KParams P) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     using L = Smem16<PX, PY>;
     constexpr int NX = kL * PX, NY = kL * PY;
     cf *sm_tw = reinterpret_cast<cf *>(smem_raw);
@@ -514,6 +563,9 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const KParams P) {
                                         // reference index (the table) does not change
     cf *sm_pwS = sm_pwH + L::kPw;       // screen factors of this CTA's rows for the NEXT row phase
     int *sm_abort = reinterpret_cast<int *>(sm_pwS + L::kPw);
+    unsigned long long *sm_mbar = reinterpret_cast<unsigned long long *>(sm_abort + 2);   // one TMA barrier per column team
+    if (threadIdx.x < 8) mbar_init(sm_mbar + threadIdx.x, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 
     for (int i = threadIdx.x; i < L::kTw; i += kThreads16) sm_tw[i] = P.tw256[i];
     for (int i = threadIdx.x; i < (PX - 1) * kL; i += kThreads16) sm_twcx[i] = P.twcx[i];
@@ -557,7 +609,7 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const KParams P) {
         // largest live |kx bin| of the step whose column phase wrote / will read the field
         const int Fa = Fa_next, Fb = Fb_next;
         if (d.is_row) run_phase16<PX, 1, true, NX, NY, BATCH>(P, d, sm_tw, sm_twcx, sm_y, sm_pwS, tagS, ucR, Fa, Fb, CWC);
-        else run_phase16<PY, CWC, false, NX, NY, BATCH>(P, d, sm_tw, sm_twcy, sm_y, sm_pwH, tagH, ucC, Fa, Fa, CWC);
+        else run_phase16<PY, CWC, false, NX, NY, BATCH>(P, d, sm_tw, sm_twcy, sm_y, sm_pwH, tagH, ucC, Fa, Fa, CWC, sm_mbar);
         if (tracer) tr[1] = clock64();
         if (BATCH && d.is_row && d.kind == 1 && P.inten != nullptr && !(P.flags & 2u) && P.B > 1)
             tagH.src = nullptr;                // the intensity sums used the propagator buffer
