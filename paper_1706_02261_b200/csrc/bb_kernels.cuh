@@ -411,7 +411,7 @@ struct SmemLayout {
 
 template <int TX, int TY, int CW>
 __global__ void __launch_bounds__(kThreads, 1) bpm_kernel(const KParams P) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     using L = SmemLayout<TX, TY, CW>;
     cf *sm_twx = reinterpret_cast<cf *>(smem_raw);
     cf *sm_twy = sm_twx + 32 * TX;

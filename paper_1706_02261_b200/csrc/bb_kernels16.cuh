@@ -359,9 +359,9 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
     const ClassSync<16 * CW> tsync{P == 1 ? 1 + tm.team : 1 + TM::NTEAM + (int)threadIdx.x / (16 * CW)};
     static_assert(ROW || ((16 * CW) % 32 == 0 && (P == 1 ? TM::NTEAM : TM::NTEAM + kThreads16 / (16 * CW)) <= 15), "barrier ids");
 
-#pragma unroll 1
     const int k0 = BATCH ? (ROW ? a0 * B : (int)(((long long)NU * B * blockIdx.x) / gridDim.x)) : a0;
     const int k1 = BATCH ? (ROW ? a1 * B : (int)(((long long)NU * B * (blockIdx.x + 1)) / gridDim.x)) : a1;
+#pragma unroll 1
     for (int k = k0 + tm.team; k < k1; k += TM::NTEAM) {
         const int m = BATCH ? k / B : k, b = BATCH ? k - m * B : 0;
         const int u = ROW ? m : (!BATCH && k == k0 + tm.team ? uc.u0 : LV(Fin, NX, CWL).tile(m));
@@ -493,6 +493,7 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
             tm.sync();                                      // region free again for the transposes
             if constexpr (ROW) subline_fft<S2, CW>(v, sm_tw, ybuf, tm.t, hsync);
             else subline_fft<S2, CW>(v, sm_tw, ybuf, tm.t, tsync);
+            // (a TMA store of the tile, the mirror image of its load, was slower: the team waits for its completion)
             cf *dst = line + tm.c * CS + tm.t * IS;
 #pragma unroll
             for (int i = 0; i < 16; ++i) st_cg(dst + 16 * IS * i, v[i]);     // dead columns too: predicated
