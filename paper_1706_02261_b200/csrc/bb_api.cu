@@ -319,16 +319,16 @@ EncodeTiledFn encode_tiled_fn() {
     }
     return fn;
 }
-// field [Ny][Nx] of 8-byte elements as (column, y mod PY, y div PY); box = (cw, 1, 256)
-bool make_field_tmap(CUtensorMap *tm, void *field, int Nx, int Ny, int cw) {
+// fields [B][Ny][Nx] of 8-byte elements as (column, y mod PY, y div PY, field); box = (cw, 1, 256, 1)
+bool make_field_tmap(CUtensorMap *tm, void *field, int Nx, int Ny, int B, int cw) {
     EncodeTiledFn fn = encode_tiled_fn();
     if (!fn || getenv("BB_K16_NOTMA")) return false;
     const int PY = Ny / 256;
-    cuuint64_t dims[3] = {(cuuint64_t)Nx, (cuuint64_t)PY, 256};
-    cuuint64_t strides[2] = {(cuuint64_t)Nx * 8, (cuuint64_t)PY * Nx * 8};
-    cuuint32_t box[3] = {(cuuint32_t)cw, 1, 256};
-    cuuint32_t estr[3] = {1, 1, 1};
-    return fn(tm, CU_TENSOR_MAP_DATA_TYPE_UINT64, 3, field, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+    cuuint64_t dims[4] = {(cuuint64_t)Nx, (cuuint64_t)PY, 256, (cuuint64_t)B};
+    cuuint64_t strides[3] = {(cuuint64_t)Nx * 8, (cuuint64_t)PY * Nx * 8, (cuuint64_t)Nx * Ny * 8};
+    cuuint32_t box[4] = {(cuuint32_t)cw, 1, 256, 1};
+    cuuint32_t estr[4] = {1, 1, 1, 1};
+    return fn(tm, CU_TENSOR_MAP_DATA_TYPE_UINT64, 4, field, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
@@ -363,7 +363,7 @@ int launch_steps(Plan *p, cf *field, const float *dn, float *inten, long long in
     P.fmax = p->d_fmax; P.cw4 = p->cw4;
     P.flags = flags & 3u;
     const bool k16 = use_k16(p, B);
-    if (k16 && B == 1) P.use_tma = make_field_tmap(&P.tmap, field, p->Nx, p->Ny, p->cw4 ? 4 : 8) ? 1 : 0;
+    if (k16) P.use_tma = make_field_tmap(&P.tmap, field, p->Nx, p->Ny, B, p->cw4 ? 4 : 8) ? 1 : 0;
     if (g_trace && k16 && 2 * j1 + 1 <= g_trace_phases) { P.trace = g_trace; P.trace_p0 = 0; }
     auto launch = [&](bool coop) {
         return k16 ? bb::kernel16_launch(p->Nx, p->Ny, P, p->grid, coop, s)

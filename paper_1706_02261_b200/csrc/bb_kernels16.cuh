@@ -179,9 +179,10 @@ __device__ __forceinline__ bool mbar_wait(unsigned long long *bar, unsigned pari
     }
     return false;
 }
-__device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *tm, int c0, int c1, int c2, unsigned long long *bar) {
-    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-                 ::"r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *tm, int c0, int c1, int c2, int c3,
+                                            unsigned long long *bar) {
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+                 ::"r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
 }
 
 struct HalfWarpSync {
@@ -374,7 +375,7 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
         cf *line = K.field + b * npx + (ROW ? (long long)u * NX : (long long)u * CW + tm.col);
         cf v[16];
         bool loaded = false;
-        if constexpr (!ROW && !BATCH) {
+        if constexpr (!ROW) {
             if (K.use_tma) {
                 // One thread asks the TMA unit for the P y-classes of the tile ([256][CW] each, into the
                 // team's part of the transpose region); the 16 CW strided 8 CW-byte row segments per warp
@@ -385,7 +386,7 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
                     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                     mbar_expect_tx(bar, (unsigned)(P * kL * CW * sizeof(cf)));
 #pragma unroll
-                    for (int cc = 0; cc < P; ++cc) tma_load_3d(stage + cc * kL * CW, &K.tmap, u * CW, cc, 0, bar);
+                    for (int cc = 0; cc < P; ++cc) tma_load_4d(stage + cc * kL * CW, &K.tmap, u * CW, cc, 0, b, bar);
                 }
                 if (!mbar_wait(bar, uc.tma_parity)) atomicExch(K.status, 2);
                 uc.tma_parity ^= 1u;
