@@ -192,6 +192,26 @@ def test_more_reference_indices_than_cached_tables(oracle_mod, monkeypatch):
     assert rel_l2(u, uo) < small_tol(7) and rel_l2(I, Io) < 2 * small_tol(7)
 
 
+@pytest.mark.parametrize("env", ["BB_K16_NOTMA", "BB_K16_NOPRUNE", "BB_DISABLE_K16"])
+def test_diagnostic_switches_do_not_change_results(oracle_mod, monkeypatch, env):
+    """The plain-load path behind the TMA tile loads, the unpruned path and the 32-point-thread kernel
+    stay exercised: same oversampled problem, each switch on, against the oracle."""
+    bb = need_gpu()
+    w = wl.tiny(N=512, Nz=6, n_cells=10, r_lo=0.5, r_hi=3.0)
+    w = wl.dataclasses.replace(w, Ny=1024, dx=0.09)
+    dn = wl.make_dn(w)
+    f0 = wl.random_field(w.Nx, w.Ny, seed=21, batch=1)
+    nref = np.linspace(1.30, 1.42, w.Nz).astype(np.float32)
+    monkeypatch.setenv(env, "1")
+    bb.shutdown()
+    try:
+        u, I, uo, Io = run_both(bb, oracle_mod, w, dn, f0, nref)
+    finally:
+        monkeypatch.delenv(env)
+        bb.shutdown()
+    assert rel_l2(u, uo) < small_tol(w.Nz) and rel_l2(I, Io) < 2 * small_tol(w.Nz)
+
+
 def test_host_buffer_entry_point_with_a_batch(oracle_mod):
     """Host buffers, B = 3 fields on a 256 x 512 grid (batch variant of the 16-point-thread kernel),
     dn streamed in several chunks; summed intensity (shared-memory atomics: compared to tolerance)."""
