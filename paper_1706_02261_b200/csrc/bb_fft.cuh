@@ -84,8 +84,6 @@ __device__ __forceinline__ constexpr double sin32d(int m) {   // sin(2 pi m/32) 
 __device__ __forceinline__ constexpr float hi_of(double c) { return (float)c; }
 __device__ __forceinline__ constexpr float lo_of(double c) { return (float)(c - (double)(float)c); }
 
-// t * r for a two-float constant r = rh + rl: one rounding of t*rh + t*rl.
-__device__ __forceinline__ float mul_hilo(float t, float rh, float rl) { return fmaf(t, rh, t * rl); }
 
 // a * exp(SIGN * 2 pi i * M / 32),  0 <= M < 16.
 // The constants are two-float values and the low parts enter INSIDE the fused multiply-add

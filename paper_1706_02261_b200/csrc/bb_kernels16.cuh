@@ -23,7 +23,6 @@
 namespace bb {
 
 constexpr int kThreads16 = 512;
-constexpr int kCW16 = 8;                       // columns per column tile: 64-byte row segments
 
 template <int PX, int PY>
 struct Smem16 {
@@ -137,14 +136,13 @@ struct LiveCols {
 // tau < lo or tau >= hi with tau = (e0 + 16 i) >> cw_log2 = (i << (4 - cw_log2)) + (e0 >> cw_log2).
 template <int P>
 __device__ __forceinline__ unsigned live_mask16(int F, int N, int c, int e0, int cw_log2) {
-    const int L = N / P, cw = 1 << cw_log2, ntc = L >> cw_log2;
+    const int L = N / P, cw = 1 << cw_log2;
     int lo_cols = F >= c ? (F - c) / P + 1 : 0;
     if (lo_cols > L) lo_cols = L;
     int hs = (N - F - c + P - 1) / P;
     if (hs > L) hs = L;
     int lo = (lo_cols + cw - 1) >> cw_log2, hi = hs >> cw_log2;
     if (lo >= hi) return 0xFFFFu;
-    (void)ntc;
     const int sh = 4 - cw_log2, t2 = e0 >> cw_log2, r = (1 << sh) - 1;
     int nl = (lo - t2 + r) >> sh, nh = (hi - t2 + r) >> sh;        // i < nl or i >= nh
     nl = nl < 0 ? 0 : (nl > 16 ? 16 : nl);
@@ -300,11 +298,11 @@ __device__ __forceinline__ void stage_rows_screen(const KParams &K, const Phase1
 
 // ----------------------------------------------------------------------------------------
 // One phase over the lines (rows, or tiles of CW columns) this CTA owns.
-//   ROW : P = PX, CW = 1, signs (+1, -1);  column: P = PY, CW = kCW16, signs (-1, +1).
+//   ROW : P = PX, CW = 1, signs (+1, -1);  column: P = PY, CW = 8 or 4, signs (-1, +1).
 // ----------------------------------------------------------------------------------------
 template <int P, int CW, bool ROW, int NX, int NY, bool BATCH>
 __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, const cf *sm_tw, const cf *sm_twc,
-                                            cf *sm_y, cf *sm_pw, PwTag &tag, UnitCache &uc, int Fin, int Fout, int cwc,
+                                            cf *sm_y, cf *sm_pw, PwTag &tag, UnitCache &uc, int Fin, int cwc,
                                             unsigned long long *sm_mbar = nullptr) {
     typedef Team16<P, CW> TM;
     constexpr int S1 = ROW ? +1 : -1, S2 = -S1;
@@ -330,7 +328,6 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
     const int a0 = uc.a0, a1 = uc.a1;
     const unsigned lmask = uc.lmask;
     const int NU = ROW ? NY : (BATCH ? LV(Fin, NX, CWL).total() : 0);
-    (void)Fout;
     cf *ybuf = sm_y + ((threadIdx.x / (16 * CW)) * (16 * 17 * CW)) + tm.col;        // one region per (team, class)
     cf *xbuf = sm_y + tm.team * (TM::TEAM * 17) + tm.col;                            // same memory, team's part
     cf *pw = sm_pw + threadIdx.x;
@@ -576,17 +573,13 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const __grid_const
 
     PwTag tagH = {nullptr, -1}, tagS = {nullptr, -1};
     UnitCache ucR, ucC;
-    // largest live |kx bin| of the step whose column phase wrote (Fa) / will read (Fb) the field of a
-    // phase; fetched one phase ahead so that the global load is not on the critical path
+    // largest live |kx bin| of the step whose column phase wrote the field a phase reads (row phase)
+    // or whose tiles it computes (column phase); fetched one phase ahead so that the global load is not on the critical path
     auto live_in = [&](int p) {
         const bool row = (p & 1) == 0;
         return row ? ((p >> 1) >= 1 ? P.fmax[(p >> 1) - 1] : NX / 2) : P.fmax[p >> 1];
     };
-    auto live_out = [&](int p) {
-        const bool row = (p & 1) == 0;
-        return row ? ((p >> 1) < P.Nz_total ? P.fmax[p >> 1] : NX / 2) : P.fmax[p >> 1];
-    };
-    int Fa_next = live_in(P.p0), Fb_next = live_out(P.p0);
+    int Fa_next = live_in(P.p0);
     Phase16 d_next = decode_phase16(P, P.p0);
     const int r0 = (int)((unsigned)NY * blockIdx.x / gridDim.x);          // rows of this CTA (row phases)
     const int r1 = (int)((unsigned)NY * (blockIdx.x + 1) / gridDim.x);
@@ -609,9 +602,9 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const __grid_const
             }
         }
         // largest live |kx bin| of the step whose column phase wrote / will read the field
-        const int Fa = Fa_next, Fb = Fb_next;
-        if (d.is_row) run_phase16<PX, 1, true, NX, NY, BATCH>(P, d, sm_tw, sm_twcx, sm_y, sm_pwS, tagS, ucR, Fa, Fb, CWC);
-        else run_phase16<PY, CWC, false, NX, NY, BATCH>(P, d, sm_tw, sm_twcy, sm_y, sm_pwH, tagH, ucC, Fa, Fa, CWC, sm_mbar);
+        const int Fa = Fa_next;
+        if (d.is_row) run_phase16<PX, 1, true, NX, NY, BATCH>(P, d, sm_tw, sm_twcx, sm_y, sm_pwS, tagS, ucR, Fa, CWC);
+        else run_phase16<PY, CWC, false, NX, NY, BATCH>(P, d, sm_tw, sm_twcy, sm_y, sm_pwH, tagH, ucC, Fa, CWC, sm_mbar);
         if (tracer) tr[1] = clock64();
         if (BATCH && d.is_row && d.kind == 1 && P.inten != nullptr && !(P.flags & 2u) && P.B > 1)
             tagH.src = nullptr;                // the intensity sums used the propagator buffer
@@ -620,7 +613,6 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const __grid_const
             grid_arrive(P.bar);
             if (tracer) tr[2] = clock64();
             Fa_next = live_in(p + 1);
-            Fb_next = live_out(p + 1);
             d_next = decode_phase16(P, p + 1);   // its global loads (table pointer, phase offset) overlap the barrier
             // While the barrier is pending, stage what does not depend on the field.  After a row
             // phase: the propagator values of the coming column phase (only when the table changed)
