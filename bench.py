@@ -51,13 +51,18 @@ def measured_peaks():
 
 
 def committed_dram_traffic(workload: str):
-    """DRAM bytes per launch of the persistent kernel from the committed ncu capture, or None."""
-    p = os.path.join(ROOT, "profiles", "dram_traffic.json")
+    """DRAM bytes per launch of the persistent kernel from the committed ncu capture
+    (profiles/dram_traffic.csv; the command that made it is in the file it names), or None."""
+    import csv
+    p = os.path.join(ROOT, "profiles", "dram_traffic.csv")
     try:
         with open(p) as f:
-            return json.load(f).get(workload, {}).get("dram_bytes_per_launch")
+            for row in csv.DictReader(f):
+                if row["workload"] == workload:
+                    return int(row["dram_bytes_per_launch"])
     except Exception:
-        return None
+        pass
+    return None
 
 
 def algorithmic_per_step(w: wl.Workload, per_field_intensity=False):
