@@ -33,26 +33,26 @@ __device__ __forceinline__ cf csub(cf a, cf b) {
     return *reinterpret_cast<cf *>(&r);
 }
 // Packed-pair plumbing: ptxas folds the pair construction into operand selectors (scalar broadcast
-// R.F32, swapped halves R.F32x2.LO_HI), so these cost no instructions.
+// R.F32, swapped halves R.F32x2.LO_HI, and a sign per half: -R.F32x2.LO_HI.NP), so these cost no instructions.
 typedef unsigned long long u64;
 __device__ __forceinline__ u64 pk2(float lo, float hi) { u64 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
 __device__ __forceinline__ cf up2(u64 v) { cf r; asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v)); return r; }
+__device__ __forceinline__ u64 mul2(u64 a, u64 b) { u64 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ u64 add2(u64 a, u64 b) { u64 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { u64 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
 // (A, B) * (rh + rl) per lane, one rounding of t*rh + t*rl each: two packed instructions
-__device__ __forceinline__ cf mul_hilo2(float A, float B, float rh, float rl) {
-    u64 t, r;
-    const u64 ab = pk2(A, B);
-    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(t) : "l"(ab), "l"(pk2(rl, rl)));
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(ab), "l"(pk2(rh, rh)), "l"(t));
-    return up2(r);
+__device__ __forceinline__ cf mul_hilo2(u64 ab, float rh, float rl) {
+    return up2(fma2(ab, pk2(rh, rh), mul2(ab, pk2(rl, rl))));
 }
 
-// a * w
+// a * w as FMUL2 + FFMA2: (x c, y c) + (y, x) * (-s, s); the swapped and half-negated operand is an
+// operand selector of the instruction, not an instruction.
 __device__ __forceinline__ cf cmul(cf a, cf w) {
-    return make_float2(fmaf(a.x, w.x, -(a.y * w.y)), fmaf(a.x, w.y, a.y * w.x));
+    return up2(fma2(pk2(a.y, a.x), pk2(-w.y, w.y), mul2(pk2(a.x, a.y), pk2(w.x, w.x))));
 }
 // a * conj(w)
 __device__ __forceinline__ cf cmulc(cf a, cf w) {
-    return make_float2(fmaf(a.x, w.x, a.y * w.y), fmaf(a.y, w.x, -(a.x * w.y)));
+    return up2(fma2(pk2(a.y, a.x), pk2(w.y, -w.y), mul2(pk2(a.x, a.y), pk2(w.x, w.x))));
 }
 
 // cos(2 pi m / 32), m = 0..16, in double; the kernels use it as a two-float constant
@@ -99,17 +99,23 @@ __device__ __forceinline__ cf mul_w32(cf a) {
         return SIGN < 0 ? make_float2(a.y, -a.x) : make_float2(-a.y, a.x);
     } else if constexpr (M == 4 || M == 12) {   // * (+-1 + SIGN i)/sqrt2
         constexpr float rh = hi_of(cos32d(4)), rl = lo_of(cos32d(4));
-        const float p = a.x + a.y, q = a.y - a.x;       // p = x + y, q = y - x
+        // (p, q) = (x + y, y - x) as one packed add of (x, y) and (y, -x)
+        const u64 axy = pk2(a.x, a.y);
         if constexpr (M == 4)
-            return SIGN < 0 ? mul_hilo2(p, q, rh, rl) : mul_hilo2(-q, p, rh, rl);
+            return SIGN < 0 ? mul_hilo2(add2(axy, pk2(a.y, -a.x)), rh, rl)        // ( p,  q)
+                            : mul_hilo2(add2(axy, pk2(-a.y, a.x)), rh, rl);       // (-q,  p)
         else
-            return SIGN < 0 ? mul_hilo2(q, -p, rh, rl) : mul_hilo2(-p, -q, rh, rl);
+            return SIGN < 0 ? mul_hilo2(add2(pk2(-a.x, -a.y), pk2(a.y, -a.x)), rh, rl)   // ( q, -p)
+                            : mul_hilo2(add2(pk2(-a.x, -a.y), pk2(-a.y, a.x)), rh, rl);  // (-p, -q)
     } else {
+        // a * (c + i s), c = ch + cl, s = sh + sl: four packed instructions, low parts first
         constexpr double cd = cos32d(M), sd = SIGN < 0 ? -sin32d(M) : sin32d(M);
         constexpr float c = hi_of(cd), cl = lo_of(cd), s = hi_of(sd), sl = lo_of(sd);
-        const float lre = fmaf(a.x, cl, -(a.y * sl));
-        const float lim = fmaf(a.x, sl, a.y * cl);
-        return make_float2(fmaf(a.x, c, fmaf(-a.y, s, lre)), fmaf(a.x, s, fmaf(a.y, c, lim)));
+        const u64 axy = pk2(a.x, a.y), ayx = pk2(a.y, a.x);
+        u64 t = mul2(ayx, pk2(-sl, sl));
+        t = fma2(axy, pk2(cl, cl), t);
+        t = fma2(ayx, pk2(-s, s), t);
+        return up2(fma2(axy, pk2(c, c), t));
     }
 }
 
