@@ -328,6 +328,49 @@ def time_batch_workload(bb, dev, steps=3):
             "propagate_ms": ms, "value": w.batch * w.Nx * w.Ny * w.Nz / (ms * 1e-3) / 1e6, "unit": "Mvox/s"}
 
 
+def run_trace(args):
+    """Per-phase timeline of the persistent kernel (bb_probe_trace) on the first N z-steps of the
+    workload: medians over CTAs and steps of work / arrive / staging / wait, per phase kind."""
+    from paper_1706_02261_b200 import binding as bb, build
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    build.build_library()
+    bb.load()
+    w = wl.config(args.workload).with_nz(args.trace)
+    dn, f0, em = make_inputs(w, dev)
+    nref = bb.nref_from_dn(dn, w.n0, w.nref_slab).numpy()
+    if em is not None:
+        field0 = bb.multiplex_psf(*(t.to(dev) for t in em), w.NA, w.Nx, w.Ny, w.dx, w.lam)[None]
+    else:
+        field0 = torch.from_numpy(f0).to(dev)
+    inten = torch.empty((w.Nz, w.Ny, w.Nx), dtype=torch.float32, device=dev)
+    grid = torch.cuda.get_device_properties(dev).multi_processor_count
+    phases = 2 * w.Nz + 1
+    buf = torch.zeros((phases, grid, 6), dtype=torch.int64, device=dev)
+    for it in range(3):
+        field = field0.clone()
+        if it == 2:
+            bb.probe_trace(buf)
+        bb.propagate(field, dn, w.dx, w.dz, w.lam, w.n0, intensity=inten, nref=nref)
+        torch.cuda.synchronize()
+    bb.probe_trace(None)
+    t = buf.cpu().numpy().astype(np.float64)
+    if not t[1:-1, :, 4].all():
+        raise SystemExit("no trace recorded: this shape / batch does not run the traced kernel")
+    # SM cycles per microsecond from the global timer (ns) at release of consecutive phases
+    cyc_per_us = np.median((t[2:-1, :, 4] - t[1:-2, :, 4]) / np.maximum(t[2:-1, :, 5] - t[1:-2, :, 5], 1.0)) * 1e3
+    out = {"workload": w.name, "z_steps": w.Nz, "sm_cycles_per_us": cyc_per_us, "unit": "us (median over CTAs and steps)"}
+    for name, sel in (("row_phase", slice(2, phases - 1, 2)), ("column_phase", slice(1, phases - 1, 2))):
+        p = t[sel]
+        seg = {"work": p[:, :, 1] - p[:, :, 0], "arrive": p[:, :, 2] - p[:, :, 1],
+               "staging": p[:, :, 3] - p[:, :, 2], "wait": p[:, :, 4] - p[:, :, 3], "total": p[:, :, 4] - p[:, :, 0]}
+        out[name] = {k: float(np.median(v) / cyc_per_us) for k, v in seg.items()}
+        out[name]["work_max_over_ctas"] = float(np.median(seg["work"].max(axis=1)) / cyc_per_us)
+    rel = t[1:-1, :, 5].max(axis=1)
+    out["us_per_z_step"] = float(np.median(rel[2:] - rel[:-2]) * 1e-3)
+    print(json.dumps(out))
+
+
 def oracle_sample(w, dn, f0, em, nref, budget_s=15.0, slices=None):
     """Times the oracle, as it stands, on the first `slices` z-slices of the workload."""
     import oracle
@@ -409,12 +452,16 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-probe", action="store_true")
     ap.add_argument("--no-batch", action="store_true", help="skip the C5 batched-fields timing")
+    ap.add_argument("--trace", type=int, default=0, metavar="N",
+                    help="print the per-phase timeline of the persistent kernel over the first N z-steps and exit")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours" and not args.nz:
         args.warmup = 3                                   # timing rule: at least 3 warm-up steps
-    if args.impl == "reference":
+    if args.trace:
+        run_trace(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
