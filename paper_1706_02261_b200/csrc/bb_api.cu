@@ -70,6 +70,8 @@ struct Plan {
     cf *twx = nullptr, *twy = nullptr;
     cf *tw256 = nullptr, *twcx = nullptr, *twcy = nullptr;   // 16-point-thread kernel tables
     bool k16 = false;              // that kernel is available for this shape
+    bool k8 = false;               // 8-point-thread kernel available for this shape
+    bool k32 = false;              // 32-point-thread kernel (all shapes up to 1024; transform programs)
     unsigned *bar = nullptr;
     int *status = nullptr;
     std::vector<TableEntry> tables;
@@ -129,16 +131,20 @@ int get_plan(int Nx, int Ny, Plan **out) {
         if (p->device == dev && p->Nx == Nx && p->Ny == Ny) { *out = p; return BB_OK; }
     Plan *p = new Plan();
     p->device = dev; p->Nx = Nx; p->Ny = Ny; p->sm_count = sms;
-    std::vector<cf> tx = make_twiddles(Nx), ty = make_twiddles(Ny);
-    BB_CUDA(cudaMalloc(&p->twx, tx.size() * sizeof(cf)));
-    BB_CUDA(cudaMalloc(&p->twy, ty.size() * sizeof(cf)));
-    BB_CUDA(cudaMemcpy(p->twx, tx.data(), tx.size() * sizeof(cf), cudaMemcpyHostToDevice));
-    BB_CUDA(cudaMemcpy(p->twy, ty.data(), ty.size() * sizeof(cf), cudaMemcpyHostToDevice));
+    if (Nx <= 1024 && Ny <= 1024) {
+        std::vector<cf> tx = make_twiddles(Nx), ty = make_twiddles(Ny);
+        BB_CUDA(cudaMalloc(&p->twx, tx.size() * sizeof(cf)));
+        BB_CUDA(cudaMalloc(&p->twy, ty.size() * sizeof(cf)));
+        BB_CUDA(cudaMemcpy(p->twx, tx.data(), tx.size() * sizeof(cf), cudaMemcpyHostToDevice));
+        BB_CUDA(cudaMemcpy(p->twy, ty.data(), ty.size() * sizeof(cf), cudaMemcpyHostToDevice));
+    }
     BB_CUDA(cudaMalloc(&p->bar, 256));
     BB_CUDA(cudaMalloc(&p->status, 256));
     BB_CUDA(cudaMemset(p->bar, 0, 256));
     BB_CUDA(cudaMemset(p->status, 0, 256));
-    if (bb::kernel16_supports(Nx, Ny) && !getenv("BB_DISABLE_K16")) {
+    const bool want16 = bb::kernel16_supports(Nx, Ny) && !getenv("BB_DISABLE_K16");
+    const bool want8 = bb::kernel8_supports(Nx, Ny) && !getenv("BB_DISABLE_K8");
+    if (want16 || want8) {
         // sub-line twiddles exp(-2 pi i k1 t / 256) and class twiddles exp(-2 pi i c q / N), c = 1..P-1, q < 256
         std::vector<cf> t256(256);
         for (int k1 = 0; k1 < 16; ++k1)
@@ -163,17 +169,29 @@ int get_plan(int Nx, int Ny, Plan **out) {
         BB_CUDA(cudaMemcpy(p->tw256, t256.data(), t256.size() * sizeof(cf), cudaMemcpyHostToDevice));
         BB_CUDA(cudaMemcpy(p->twcx, cx.data(), cx.size() * sizeof(cf), cudaMemcpyHostToDevice));
         BB_CUDA(cudaMemcpy(p->twcy, cy.data(), cy.size() * sizeof(cf), cudaMemcpyHostToDevice));
-        int rc16 = bb::kernel16_prepare(Nx, Ny);
-        if (rc16 != 0) { delete p; return fail(BB_ERR_CUDA, "kernel16_prepare failed: %s", cudaGetErrorString((cudaError_t)rc16)); }
-        if (bb::kernel16_blocks_per_sm(Nx, Ny) < 1) { delete p; return fail(BB_ERR_CUDA, "16-point BPM kernel does not fit on an SM"); }
-        p->k16 = true;
+        if (want16) {
+            int rc16 = bb::kernel16_prepare(Nx, Ny);
+            if (rc16 != 0) { delete p; return fail(BB_ERR_CUDA, "kernel16_prepare failed: %s", cudaGetErrorString((cudaError_t)rc16)); }
+            if (bb::kernel16_blocks_per_sm(Nx, Ny) < 1) { delete p; return fail(BB_ERR_CUDA, "16-point BPM kernel does not fit on an SM"); }
+            p->k16 = true;
+        }
+        if (want8) {
+            int rc8 = bb::kernel8_prepare(Nx, Ny);
+            if (rc8 != 0) { delete p; return fail(BB_ERR_CUDA, "kernel8_prepare failed: %s", cudaGetErrorString((cudaError_t)rc8)); }
+            if (bb::kernel8_blocks_per_sm(Nx, Ny) < 1) { delete p; return fail(BB_ERR_CUDA, "8-point BPM kernel does not fit on an SM"); }
+            p->k8 = true;
+        }
     }
     size_t tb = (size_t)Nx * Ny * sizeof(cf);
     p->table_capacity = std::max<size_t>(2, std::min<size_t>(4096, table_budget_bytes() / tb));
-    rc = bb::kernel_prepare(Nx, Ny);
-    if (rc != 0) { delete p; return fail(BB_ERR_CUDA, "kernel_prepare failed: %s", cudaGetErrorString((cudaError_t)rc)); }
-    int per_sm = bb::kernel_blocks_per_sm(Nx, Ny);
-    if (per_sm < 1) { delete p; return fail(BB_ERR_CUDA, "BPM kernel does not fit on an SM"); }
+    if (Nx <= 1024 && Ny <= 1024) {
+        rc = bb::kernel_prepare(Nx, Ny);
+        if (rc != 0) { delete p; return fail(BB_ERR_CUDA, "kernel_prepare failed: %s", cudaGetErrorString((cudaError_t)rc)); }
+        int per_sm = bb::kernel_blocks_per_sm(Nx, Ny);
+        if (per_sm < 1) { delete p; return fail(BB_ERR_CUDA, "BPM kernel does not fit on an SM"); }
+        p->k32 = true;
+    }
+    if (!p->k32 && !p->k8) { delete p; return fail(BB_ERR_UNSUPPORTED_SHAPE, "no kernel for Nx = %d, Ny = %d", Nx, Ny); }
     p->grid = sms;
     g_plans.push_back(p);
     *out = p;
@@ -234,7 +252,8 @@ int live_tiles(int N, int F, int cw) {
 // one propagation): 4 columns when the (tile, field) units then still fit one per SM, else 8.
 void choose_tile_width(Plan *p, int B, int Nz, float dx, float lambda, float n0, const float *nref) {
     p->cw4 = 0;
-    if (!p->k16) return;
+    if (!p->k16 && !p->k8) return;
+    if (p->Ny > 1024) { p->cw4 = 1; return; }          // a tile of 8 columns x 2048 rows exceeds one team
     double k0 = kTwoPi / (double)lambda;
     int F = 0;
     for (int j = 0; j < Nz; ++j) F = std::max(F, live_fmax(p->Nx, (double)dx, k0 * (double)(nref ? nref[j] : n0)));
@@ -270,6 +289,15 @@ int get_table(Plan *p, const TableKey &k, cudaStream_t s, unsigned long long pro
     return BB_OK;
 }
 
+// Supported grids: powers of two in [32, 2048]; 2048-point lines exist only in the 8-point-thread
+// kernel, which needs both sides >= 256.
+bool shape_ok(int Nx, int Ny) {
+    const int lx = log2_exact(Nx), ly = log2_exact(Ny);
+    if (lx < 5 || lx > 11 || ly < 5 || ly > 11) return false;
+    if ((lx == 11 || ly == 11) && (lx < 8 || ly < 8)) return false;
+    return true;
+}
+
 int validate_common(const void *field, const float *dn, int Nx, int Ny, int Nz, float dx, float dz,
                     float lambda, float n0, const bb_opts *opts, int *B, unsigned *flags) {
     if (!field) return fail(BB_ERR_INVALID_ARG, "field is NULL");
@@ -278,9 +306,8 @@ int validate_common(const void *field, const float *dn, int Nx, int Ny, int Nz, 
     if (!(dx > 0.f) || !(dz > 0.f) || !(lambda > 0.f) || !(n0 > 0.f) || !std::isfinite(dx) ||
         !std::isfinite(dz) || !std::isfinite(lambda) || !std::isfinite(n0))
         return fail(BB_ERR_INVALID_ARG, "dx, dz, lambda, n0 must be positive and finite");
-    int lx = log2_exact(Nx), ly = log2_exact(Ny);
-    if (lx < 5 || lx > 10 || ly < 5 || ly > 10)
-        return fail(BB_ERR_UNSUPPORTED_SHAPE, "Nx = %d, Ny = %d: both must be powers of two in [32, 1024]", Nx, Ny);
+    if (!shape_ok(Nx, Ny))
+        return fail(BB_ERR_UNSUPPORTED_SHAPE, "Nx = %d, Ny = %d: both must be powers of two in [32, 2048], and both >= 256 if one is 2048", Nx, Ny);
     *B = 1;
     *flags = 0;
     if (opts) {
@@ -334,8 +361,13 @@ bool make_field_tmap(CUtensorMap *tm, void *field, int Nx, int Ny, int B, int cw
 
 // The 16-point-thread kernel serves single fields on 256/512/1024 grids; everything else (batches,
 // other shapes, the generic transform programs) runs on the 32-point-thread kernel.
+bool use_k8(const Plan *p, int B) {
+    if (!p->k8 || getenv("BB_USE_K16")) return false;
+    const int rows = (p->Ny + p->grid - 1) / p->grid;
+    return B == 1 || (long long)rows * p->Nx <= 8192;
+}
 bool use_k16(const Plan *p, int B) {
-    if (!p->k16) return false;
+    if (!p->k16 || use_k8(p, B)) return false;
     // the batch variant shares one buffer of screen factors among the teams: all rows of a CTA must fit
     const int rows = (p->Ny + p->grid - 1) / p->grid;
     return B == 1 || (long long)rows * p->Nx <= 8192;
@@ -362,12 +394,15 @@ int launch_steps(Plan *p, cf *field, const float *dn, float *inten, long long in
     P.tw256 = p->tw256; P.twcx = p->twcx; P.twcy = p->twcy;
     P.fmax = p->d_fmax; P.cw4 = p->cw4;
     P.flags = flags & 3u;
-    const bool k16 = use_k16(p, B);
-    if (k16) P.use_tma = make_field_tmap(&P.tmap, field, p->Nx, p->Ny, B, p->cw4 ? 4 : 8) ? 1 : 0;
-    if (g_trace && k16 && 2 * j1 + 1 <= g_trace_phases) { P.trace = g_trace; P.trace_p0 = 0; }
+    for (int i = 0; i < 4; ++i) { char nm[16]; snprintf(nm, sizeof nm, "BB_XP%d", i); const char *e = getenv(nm); P.xp[i] = e ? atoi(e) : 0; }
+    const bool k8 = use_k8(p, B), k16 = use_k16(p, B);
+    if (!k8 && !k16 && !p->k32) return fail(BB_ERR_UNSUPPORTED_SHAPE, "no kernel for Nx = %d, Ny = %d, batch = %d", p->Nx, p->Ny, B);
+    if (k16 || k8) P.use_tma = make_field_tmap(&P.tmap, field, p->Nx, p->Ny, B, p->cw4 ? 4 : 8) ? 1 : 0;
+    if (g_trace && (k16 || k8) && 2 * j1 + 1 <= g_trace_phases) { P.trace = g_trace; P.trace_p0 = 0; }
     auto launch = [&](bool coop) {
-        return k16 ? bb::kernel16_launch(p->Nx, p->Ny, P, p->grid, coop, s)
-                   : bb::kernel_launch(p->Nx, p->Ny, P, p->grid, coop, s);
+        return k8 ? bb::kernel8_launch(p->Nx, p->Ny, P, p->grid, coop, s)
+                  : k16 ? bb::kernel16_launch(p->Nx, p->Ny, P, p->grid, coop, s)
+                        : bb::kernel_launch(p->Nx, p->Ny, P, p->grid, coop, s);
     };
     int p0 = (j0 == 0) ? 0 : 2 * j0 + 1, p1 = 2 * j1 + 1;
     if (flags & BB_LAUNCH_PER_PHASE) {
@@ -400,7 +435,7 @@ int prepare_steps(Plan *p, int B, int Nz, int j0, float dx, float dz, float lamb
     for (; j < Nz; ++j) {
         float nr = nref ? nref[j] : n0;
         if (!(last_ptr && nr == last_nref)) {
-            TableKey key = {dx, dz, lambda, nr, use_k16(p, B) ? p->Nx / 256 : 1};
+            TableKey key = {dx, dz, lambda, nr, (use_k16(p, B) || use_k8(p, B)) ? p->Nx / 256 : 1};
             cf *ptr = nullptr;
             int rc = get_table(p, key, s, protect, &ptr);
             if (rc == kTableCacheFull) break;                 // the rest goes into the next launch
@@ -506,6 +541,45 @@ cudaError_t kernel16_launch(int Nx, int Ny, const KParams &P, int grid, bool coo
     } else {
         if (P.cw4) { BB_SWITCH_PX(4, 0, launch, Ny / 256, P, grid, coop, s) }
         else { BB_SWITCH_PX(8, 0, launch, Ny / 256, P, grid, coop, s) }
+    }
+    return cudaErrorInvalidValue;
+}
+#define BB_SWITCH_PX8(cw, bt, fn, ...)                               \
+    switch (Nx / 256) {                                              \
+        case 1: return inst8_1_cw##cw##_b##bt##_##fn(__VA_ARGS__);   \
+        case 2: return inst8_2_cw##cw##_b##bt##_##fn(__VA_ARGS__);   \
+        case 4: return inst8_4_cw##cw##_b##bt##_##fn(__VA_ARGS__);   \
+        case 8: return inst8_8_cw##cw##_b##bt##_##fn(__VA_ARGS__);   \
+    }
+bool kernel8_supports(int Nx, int Ny) {
+    auto ok = [](int n) { return n == 256 || n == 512 || n == 1024 || n == 2048; };
+    return ok(Nx) && ok(Ny);
+}
+int kernel8_prepare(int Nx, int Ny) {
+    auto f0 = [&]() -> cudaError_t { BB_SWITCH_PX8(8, 0, prepare, Ny / 256) return cudaErrorInvalidValue; };
+    auto f1 = [&]() -> cudaError_t { BB_SWITCH_PX8(4, 0, prepare, Ny / 256) return cudaErrorInvalidValue; };
+    auto f2 = [&]() -> cudaError_t { BB_SWITCH_PX8(8, 1, prepare, Ny / 256) return cudaErrorInvalidValue; };
+    auto f3 = [&]() -> cudaError_t { BB_SWITCH_PX8(4, 1, prepare, Ny / 256) return cudaErrorInvalidValue; };
+    cudaError_t e = f0();
+    if (e == cudaSuccess) e = f1();
+    if (e == cudaSuccess) e = f2();
+    if (e == cudaSuccess) e = f3();
+    return (int)e;
+}
+int kernel8_blocks_per_sm(int Nx, int Ny) {
+    auto f0 = [&]() -> int { BB_SWITCH_PX8(8, 0, blocks_per_sm, Ny / 256) return 0; };
+    auto f1 = [&]() -> int { BB_SWITCH_PX8(4, 0, blocks_per_sm, Ny / 256) return 0; };
+    auto f2 = [&]() -> int { BB_SWITCH_PX8(8, 1, blocks_per_sm, Ny / 256) return 0; };
+    auto f3 = [&]() -> int { BB_SWITCH_PX8(4, 1, blocks_per_sm, Ny / 256) return 0; };
+    return std::min(std::min(f0(), f1()), std::min(f2(), f3()));
+}
+cudaError_t kernel8_launch(int Nx, int Ny, const KParams &P, int grid, bool coop, cudaStream_t s) {
+    if (P.B > 1) {
+        if (P.cw4) { BB_SWITCH_PX8(4, 1, launch, Ny / 256, P, grid, coop, s) }
+        else { BB_SWITCH_PX8(8, 1, launch, Ny / 256, P, grid, coop, s) }
+    } else {
+        if (P.cw4) { BB_SWITCH_PX8(4, 0, launch, Ny / 256, P, grid, coop, s) }
+        else { BB_SWITCH_PX8(8, 0, launch, Ny / 256, P, grid, coop, s) }
     }
     return cudaErrorInvalidValue;
 }
@@ -764,9 +838,8 @@ int bb_propagator_table(int Nx, int Ny, float dx, float dz, float lambda, float 
     if (!out) return fail(BB_ERR_INVALID_ARG, "table_out is NULL");
     if (!(dx > 0.f) || !(dz > 0.f) || !(lambda > 0.f) || !(nref > 0.f))
         return fail(BB_ERR_INVALID_ARG, "dx, dz, lambda, nref must be positive");
-    int lx = log2_exact(Nx), ly = log2_exact(Ny);
-    if (lx < 5 || lx > 10 || ly < 5 || ly > 10)
-        return fail(BB_ERR_UNSUPPORTED_SHAPE, "Nx = %d, Ny = %d: both must be powers of two in [32, 1024]", Nx, Ny);
+    if (!shape_ok(Nx, Ny))
+        return fail(BB_ERR_UNSUPPORTED_SHAPE, "Nx = %d, Ny = %d: both must be powers of two in [32, 2048], and both >= 256 if one is 2048", Nx, Ny);
     Plan *p;
     int rc = get_plan(Nx, Ny, &p);
     if (rc) return rc;

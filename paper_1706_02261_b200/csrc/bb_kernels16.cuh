@@ -359,6 +359,10 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
 
     const int k0 = BATCH ? (ROW ? a0 * B : (int)(((long long)NU * B * blockIdx.x) / gridDim.x)) : a0;
     const int k1 = BATCH ? (ROW ? a1 * B : (int)(((long long)NU * B * (blockIdx.x + 1)) / gridDim.x)) : a1;
+    if (ROW && K.xp[0] > 0) {
+        const long long t0 = clock64(), dt = (long long)tm.team * K.xp[0];
+        while (clock64() - t0 < dt) {}
+    }
 #pragma unroll 1
     for (int k = k0 + tm.team; k < k1; k += TM::NTEAM) {
         const int m = BATCH ? k / B : k, b = BATCH ? k - m * B : 0;

@@ -30,6 +30,18 @@ BB_DECLARE_INST16(1, 4, 1) BB_DECLARE_INST16(2, 4, 1) BB_DECLARE_INST16(4, 4, 1)
 BB_DECLARE_INST16(1, 8, 1) BB_DECLARE_INST16(2, 8, 1) BB_DECLARE_INST16(4, 8, 1)
 #undef BB_DECLARE_INST16
 
+// 8-point-thread kernel (bb_kernels8.cuh), one set per PX = Nx/256 in {1, 2, 4, 8} and column tile width in
+// {4, 8}; bb_inst8.cu.
+#define BB_DECLARE_INST8(PX, CW, BT)                                                                              \
+    cudaError_t inst8_##PX##_cw##CW##_b##BT##_prepare(int PY);                                                     \
+    int inst8_##PX##_cw##CW##_b##BT##_blocks_per_sm(int PY);                                                       \
+    cudaError_t inst8_##PX##_cw##CW##_b##BT##_launch(int PY, const KParams &P, int grid, bool coop, cudaStream_t s);
+BB_DECLARE_INST8(1, 4, 0) BB_DECLARE_INST8(2, 4, 0) BB_DECLARE_INST8(4, 4, 0) BB_DECLARE_INST8(8, 4, 0)
+BB_DECLARE_INST8(1, 8, 0) BB_DECLARE_INST8(2, 8, 0) BB_DECLARE_INST8(4, 8, 0) BB_DECLARE_INST8(8, 8, 0)
+BB_DECLARE_INST8(1, 4, 1) BB_DECLARE_INST8(2, 4, 1) BB_DECLARE_INST8(4, 4, 1) BB_DECLARE_INST8(8, 4, 1)
+BB_DECLARE_INST8(1, 8, 1) BB_DECLARE_INST8(2, 8, 1) BB_DECLARE_INST8(4, 8, 1) BB_DECLARE_INST8(8, 8, 1)
+#undef BB_DECLARE_INST8
+
 // Dispatch on (Nx, Ny); defined in bb_api.cu.
 int kernel_prepare(int Nx, int Ny);           // returns a cudaError_t value
 int kernel_blocks_per_sm(int Nx, int Ny);
@@ -38,5 +50,9 @@ bool kernel16_supports(int Nx, int Ny);
 int kernel16_prepare(int Nx, int Ny);
 int kernel16_blocks_per_sm(int Nx, int Ny);
 cudaError_t kernel16_launch(int Nx, int Ny, const KParams &P, int grid, bool coop, cudaStream_t s);
+bool kernel8_supports(int Nx, int Ny);
+int kernel8_prepare(int Nx, int Ny);
+int kernel8_blocks_per_sm(int Nx, int Ny);
+cudaError_t kernel8_launch(int Nx, int Ny, const KParams &P, int grid, bool coop, cudaStream_t s);
 
 }  // namespace bb
