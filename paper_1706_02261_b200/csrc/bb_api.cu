@@ -72,6 +72,7 @@ struct Plan {
     bool k16 = false;              // that kernel is available for this shape
     bool k8 = false;               // 8-point-thread kernel available for this shape
     bool k32 = false;              // 32-point-thread kernel (all shapes up to 1024; transform programs)
+    bool force_k8 = false;         // BB_USE_K8=1 when the plan was made
     unsigned *bar = nullptr;
     int *status = nullptr;
     std::vector<TableEntry> tables;
@@ -180,6 +181,7 @@ int get_plan(int Nx, int Ny, Plan **out) {
             if (rc8 != 0) { delete p; return fail(BB_ERR_CUDA, "kernel8_prepare failed: %s", cudaGetErrorString((cudaError_t)rc8)); }
             if (bb::kernel8_blocks_per_sm(Nx, Ny) < 1) { delete p; return fail(BB_ERR_CUDA, "8-point BPM kernel does not fit on an SM"); }
             p->k8 = true;
+            p->force_k8 = getenv("BB_USE_K8") != nullptr;
         }
     }
     size_t tb = (size_t)Nx * Ny * sizeof(cf);
@@ -361,8 +363,11 @@ bool make_field_tmap(CUtensorMap *tm, void *field, int Nx, int Ny, int B, int cw
 
 // The 16-point-thread kernel serves single fields on 256/512/1024 grids; everything else (batches,
 // other shapes, the generic transform programs) runs on the 32-point-thread kernel.
+// 2048-point lines exist only in the 8-point-thread kernel; elsewhere the 16-point-thread kernel is
+// faster (profiles/r02_b) and the 8-point one is a diagnostic alternative (BB_USE_K8=1).
 bool use_k8(const Plan *p, int B) {
-    if (!p->k8 || getenv("BB_USE_K16")) return false;
+    if (!p->k8) return false;
+    if (p->Nx <= 1024 && p->Ny <= 1024 && p->k16 && !p->force_k8) return false;
     const int rows = (p->Ny + p->grid - 1) / p->grid;
     return B == 1 || (long long)rows * p->Nx <= 8192;
 }
@@ -394,7 +399,6 @@ int launch_steps(Plan *p, cf *field, const float *dn, float *inten, long long in
     P.tw256 = p->tw256; P.twcx = p->twcx; P.twcy = p->twcy;
     P.fmax = p->d_fmax; P.cw4 = p->cw4;
     P.flags = flags & 3u;
-    for (int i = 0; i < 4; ++i) { char nm[16]; snprintf(nm, sizeof nm, "BB_XP%d", i); const char *e = getenv(nm); P.xp[i] = e ? atoi(e) : 0; }
     const bool k8 = use_k8(p, B), k16 = use_k16(p, B);
     if (!k8 && !k16 && !p->k32) return fail(BB_ERR_UNSUPPORTED_SHAPE, "no kernel for Nx = %d, Ny = %d, batch = %d", p->Nx, p->Ny, B);
     if (k16 || k8) P.use_tma = make_field_tmap(&P.tmap, field, p->Nx, p->Ny, B, p->cw4 ? 4 : 8) ? 1 : 0;

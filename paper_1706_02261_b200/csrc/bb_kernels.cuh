@@ -57,7 +57,6 @@ struct KParams {
     int use_tma;               // 16-point-thread kernel: column tiles are fetched by TMA through `tmap`
     long long *trace;          // bb_probe_trace: [phase - trace_p0][CTA][6] time stamps, or nullptr
     int trace_p0;
-    int xp[4];                 // experiment knobs (BB_XP0..3)
     // fields as a 4-D tensor (column, y mod PY, y div PY, field) of 8-byte elements, box = (CW, 1, 256, 1):
     // one TMA request brings one y-class of a column tile, [256][CW] row-major, into shared memory
     alignas(64) CUtensorMap tmap;

@@ -231,6 +231,16 @@ __device__ __forceinline__ void screen_sincos_small(float r, float &sn, float &c
     cs = fmaf(r2 * r2, cp, fmaf(-0.5f, r2, 1.f));
 }
 
+// (cos r, sin r) for r in [-pi/4, pi/4]: the two Horner chains of screen_sincos_small as packed
+// instructions (same operations per lane, hence the same bits), for code with registers to spare.
+__device__ __forceinline__ cf screen_cossin_small_packed(float r) {
+    const float r2 = r * r;
+    u64 p = fma2(pk2(r2, r2), pk2(2.4435851735e-05f, -1.9513932562e-04f), pk2(-1.3887341487e-03f, 8.3321482563e-03f));
+    p = fma2(p, pk2(r2, r2), pk2(4.1666646237e-02f, -1.6666654339e-01f));
+    const u64 m = mul2(pk2(r2, r), pk2(r2, r2));                 // (r2 r2, r r2)
+    return up2(fma2(m, p, pk2(fmaf(-0.5f, r2, 1.f), r)));
+}
+
 // Pointwise factors of the unit the thread works on, slot (jp, m) -> pw[(jp*P + m) * kThreads16]:
 // kind 1: exp(i (pb dn + pa)) at pixel n = q(jp) + 256 m of row `unit` of a dn slice (bb.h step 4);
 // kind 2: table value H[n][column] of column tile `unit` (bb.h step 2).  Runs off the critical
@@ -296,6 +306,56 @@ __device__ __forceinline__ void stage_rows_screen(const KParams &K, const Phase1
     }
 }
 
+// Single-field kernel, column phase: a CTA that owns fewer column tiles than it has column teams (the
+// usual case on an oversampled grid, where the evanescent band is pruned: 144 live tiles on 148 SMs at
+// 1024^2) has idle warps.  They compute the screen factors exp(i (pb dn + pa)) of the CTA's rows for
+// the NEXT row phase into the thread-private columns of the row teams (slot (jp, m) of row thread
+// (team rl, class c, lane t) <- pixel n = t + 16 (PX jp + c) + 256 m of row r0 + rl), so that this
+// work leaves the critical path between two phases (profiles/r02: 1.4 us behind every row phase).
+template <int PX, int NX, int NY, int TEAMC>
+__device__ __forceinline__ void stage_screen_by_idle_warps(const KParams &K, const Phase16 &dS, cf *sm_pwS) {
+    typedef Team16<PX, 1> TR;
+    constexpr int PER = (NX + TEAMC - 1) / TEAMC;              // pixels of a row per staging thread
+    constexpr int RCH = 8;                                     // rows in flight (all loads issued before the first use)
+    const int r0 = (int)((unsigned)NY * blockIdx.x / gridDim.x);
+    const int r1 = (int)((unsigned)NY * (blockIdx.x + 1) / gridDim.x);
+    const int rows = min(r1 - r0, TR::NTEAM);
+    const int s = (int)threadIdx.x - (kThreads16 - TEAMC);     // the last column team stages
+    const float *dnp = reinterpret_cast<const float *>(dS.src) + (long long)r0 * NX + s;
+    const float pa = dS.pa, pb = K.phase_b;
+#pragma unroll 1
+    for (int rb = 0; rb < rows; rb += RCH) {
+        float x[RCH][PER];
+#pragma unroll
+        for (int rl = 0; rl < RCH; ++rl)
+#pragma unroll
+            for (int k = 0; k < PER; ++k)
+                x[rl][k] = (rb + rl < rows && s + k * TEAMC < NX) ? __ldcs(dnp + (rb + rl) * NX + k * TEAMC) : 0.f;
+#pragma unroll
+        for (int rl = 0; rl < RCH; ++rl) {
+            if (rb + rl < rows) {
+#pragma unroll
+                for (int k = 0; k < PER; ++k) {
+                    const int n = s + k * TEAMC;
+                    if (n < NX) {
+                        const int m = n >> 8, q = n & 255, t = q & 15, z = q >> 4, c = z % PX, jp = z / PX;
+                        const float a = fmaf(pb, x[rl][k], pa);
+                        cf f;
+                        if (__all_sync(__activemask(), fabsf(a) <= 0.78539816f)) {
+                            f = screen_cossin_small_packed(a);
+                        } else {
+                            float sn, cs;
+                            screen_sincos(a, sn, cs);
+                            f = make_float2(cs, sn);
+                        }
+                        sm_pwS[(jp * PX + m) * kThreads16 + (rb + rl) * TR::TEAM + c * 16 + t] = f;
+                    }
+                }
+            }
+        }
+    }
+}
+
 // ----------------------------------------------------------------------------------------
 // One phase over the lines (rows, or tiles of CW columns) this CTA owns.
 //   ROW : P = PX, CW = 1, signs (+1, -1);  column: P = PY, CW = 8 or 4, signs (-1, +1).
@@ -303,7 +363,8 @@ __device__ __forceinline__ void stage_rows_screen(const KParams &K, const Phase1
 template <int P, int CW, bool ROW, int NX, int NY, bool BATCH>
 __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, const cf *sm_tw, const cf *sm_twc,
                                             cf *sm_y, cf *sm_pw, PwTag &tag, UnitCache &uc, int Fin, int cwc,
-                                            unsigned long long *sm_mbar = nullptr) {
+                                            unsigned long long *sm_mbar = nullptr, int pstage = -1,
+                                            cf *sm_pwS = nullptr, PwTag *tagS = nullptr) {
     typedef Team16<P, CW> TM;
     constexpr int S1 = ROW ? +1 : -1, S2 = -S1;
     constexpr int JP = TM::JP;
@@ -327,6 +388,19 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
     }
     const int a0 = uc.a0, a1 = uc.a1;
     const unsigned lmask = uc.lmask;
+    if constexpr (!ROW && !BATCH) {
+        // idle column teams stage the screen factors of the next row phase (see stage_screen_by_idle_warps)
+        // pstage: the row phase after this column phase (it applies dn slice pstage / 2 - 1), or -1
+        const int busy = min(a1 - a0, TM::NTEAM);
+        const void *src_stage = pstage >= 2 ? K.dn + (long long)((pstage >> 1) - 1 - K.j_base) * ((long long)NX * NY) : nullptr;
+        if (src_stage != nullptr && busy < TM::NTEAM && tagS->src != src_stage) {
+            if (tm.team == TM::NTEAM - 1) stage_screen_by_idle_warps<NX / kL, NX, NY, TM::TEAM>(K, decode_phase16(K, pstage), sm_pwS);
+            typedef Team16<NX / kL, 1> TR;
+            const int tr = (int)threadIdx.x / TR::TEAM;
+            const int r0 = (int)((unsigned)NY * blockIdx.x / gridDim.x), r1 = (int)((unsigned)NY * (blockIdx.x + 1) / gridDim.x);
+            if (tr < TR::NTEAM && r0 + tr < r1) { tagS->src = src_stage; tagS->pix0 = r0 + tr; }
+        }
+    }
     const int NU = ROW ? NY : (BATCH ? LV(Fin, NX, CWL).total() : 0);
     cf *ybuf = sm_y + ((threadIdx.x / (16 * CW)) * (16 * 17 * CW)) + tm.col;        // one region per (team, class)
     cf *xbuf = sm_y + tm.team * (TM::TEAM * 17) + tm.col;                            // same memory, team's part
@@ -359,10 +433,6 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
 
     const int k0 = BATCH ? (ROW ? a0 * B : (int)(((long long)NU * B * blockIdx.x) / gridDim.x)) : a0;
     const int k1 = BATCH ? (ROW ? a1 * B : (int)(((long long)NU * B * (blockIdx.x + 1)) / gridDim.x)) : a1;
-    if (ROW && K.xp[0] > 0) {
-        const long long t0 = clock64(), dt = (long long)tm.team * K.xp[0];
-        while (clock64() - t0 < dt) {}
-    }
 #pragma unroll 1
     for (int k = k0 + tm.team; k < k1; k += TM::NTEAM) {
         const int m = BATCH ? k / B : k, b = BATCH ? k - m * B : 0;
@@ -607,8 +677,12 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const __grid_const
         }
         // largest live |kx bin| of the step whose column phase wrote / will read the field
         const int Fa = Fa_next;
-        if (d.is_row) run_phase16<PX, 1, true, NX, NY, BATCH>(P, d, sm_tw, sm_twcx, sm_y, sm_pwS, tagS, ucR, Fa, CWC);
-        else run_phase16<PY, CWC, false, NX, NY, BATCH>(P, d, sm_tw, sm_twcy, sm_y, sm_pwH, tagH, ucC, Fa, CWC, sm_mbar);
+        if (d.is_row) {
+            run_phase16<PX, 1, true, NX, NY, BATCH>(P, d, sm_tw, sm_twcx, sm_y, sm_pwS, tagS, ucR, Fa, CWC);
+        } else {
+            run_phase16<PY, CWC, false, NX, NY, BATCH>(P, d, sm_tw, sm_twcy, sm_y, sm_pwH, tagH, ucC, Fa, CWC, sm_mbar,
+                                                       (!BATCH && p + 1 < P.p1) ? p + 1 : -1, sm_pwS, &tagS);
+        }
         if (tracer) tr[1] = clock64();
         if (BATCH && d.is_row && d.kind == 1 && P.inten != nullptr && !(P.flags & 2u) && P.B > 1)
             tagH.src = nullptr;                // the intensity sums used the propagator buffer
@@ -626,7 +700,10 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const __grid_const
             if (d.is_row) {
                 const int Fn = Fa_next;
                 prefill_phase16<PY, CWC, false, NX, NY, BATCH>(P, d_next, sm_pwH, tagH, Fn);
-                if (p + 2 < P.p1) prefill_phase16<PX, 1, true, NX, NY, BATCH>(P, decode_phase16(P, p + 2), sm_pwS, tagS, 0);
+                // screen factors of the row phase after next: here, unless the coming column phase has
+                // idle warps for them (same live band as the last column phase, which had an idle team)
+                const bool col_stages = !BATCH && ucC.F == Fn && (ucC.a1 - ucC.a0) < Team16<PY, CWC>::NTEAM;
+                if (p + 2 < P.p1 && !col_stages) prefill_phase16<PX, 1, true, NX, NY, BATCH>(P, decode_phase16(P, p + 2), sm_pwS, tagS, 0);
             } else {
                 prefill_phase16<PX, 1, true, NX, NY, BATCH>(P, d_next, sm_pwS, tagS, 0);
             }
