@@ -21,4 +21,10 @@ from .bpm_oracle import (  # noqa: F401
     multiplex_psf,
     nref_from_dn,
     num_threads,
+    propagate_backward,
+    refocus,
+    extract_tiles,
+    lightsheet,
+    multiplex_annular,
+    image_formation,
 )

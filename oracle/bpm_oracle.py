@@ -61,6 +61,19 @@ def _load():
                                              ctypes.c_int, ctypes.c_int, ctypes.c_float, ctypes.c_float, _f64p]
         lib.oracle_nref_from_dn.argtypes = [_f32p, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                             ctypes.c_float, ctypes.c_int, _f32p]
+        lib.oracle_propagate_backward.argtypes = [_f32p, _f32p, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                                  ctypes.c_float, ctypes.c_float, ctypes.c_float, ctypes.c_float,
+                                                  _f32p, _f64p, _f64p]
+        lib.oracle_refocus.argtypes = [_f64p, ctypes.c_int, ctypes.c_int, ctypes.c_float, ctypes.c_float,
+                                       ctypes.c_float, ctypes.c_float]
+        lib.oracle_extract_tiles.argtypes = [_f64p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, _f32p,
+                                             ctypes.c_int, ctypes.c_float, ctypes.c_int, _f64p]
+        lib.oracle_lightsheet.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_float, ctypes.c_float, ctypes.c_float,
+                                          ctypes.c_float, ctypes.c_float, _f64p]
+        lib.oracle_multiplex_annular.argtypes = [_f32p, _f32p, _f32p, ctypes.c_int, ctypes.c_float, ctypes.c_float,
+                                                 ctypes.c_int, ctypes.c_int, ctypes.c_float, ctypes.c_float, _f64p]
+        lib.oracle_image_formation.argtypes = [_f64p, ctypes.c_int, ctypes.c_int, _f32p, ctypes.c_int, ctypes.c_float,
+                                               _f64p, ctypes.c_int, _f64p]
         _lib = lib
         return lib
 
@@ -229,4 +242,77 @@ def nref_from_dn(dn, n0, slab) -> np.ndarray:
     out = np.empty((Nz,), dtype=np.float32)
     _check(_load().oracle_nref_from_dn(_p32(dn), Nx, Ny, Nz, _sf(n0), int(slab), _p32(out)),
            "oracle_nref_from_dn")
+    return out
+
+
+def propagate_backward(field, dn, dx, dz, lam, n0, nref=None, want_intensity=True):
+    """Time-reversed propagation (``oracle_propagate_backward``): returns (field at z = 0, I[Nz][Ny][Nx] or None)."""
+    f = np.ascontiguousarray(field, dtype=np.complex64)
+    Ny, Nx = f.shape
+    dn = _f32(dn)
+    Nz = dn.shape[0]
+    nref = _f32(nref, (Nz,))
+    out = np.empty((Ny, Nx), dtype=np.complex128)
+    I = np.empty((Nz, Ny, Nx), dtype=np.float64) if want_intensity else None
+    rc = _load().oracle_propagate_backward(f.view(np.float32).ctypes.data_as(_f32p), _p32(dn), Nx, Ny, Nz,
+                                           _sf(dx), _sf(dz), _sf(lam), _sf(n0), _p32(nref), _p64(out),
+                                           None if I is None else _p64(I))
+    _check(rc, "oracle_propagate_backward")
+    return out, I
+
+
+def refocus(u, dx, dz, lam, n) -> np.ndarray:
+    """One homogeneous-medium step of SIGNED length dz (``oracle_refocus``)."""
+    u = _c128(u)
+    Ny, Nx = u.shape
+    _check(_load().oracle_refocus(_p64(u), Nx, Ny, _sf(dx), _sf(dz), _sf(lam), _sf(n)), "oracle_refocus")
+    return u
+
+
+def extract_tiles(src, pos, dx, T) -> np.ndarray:
+    """T x T windows around the emitters of every plane of ``src`` ([Np][Ny][Nx] or [Ny][Nx], real or
+    complex): returns [M][Np][T][T] (``oracle_extract_tiles``)."""
+    a = np.asarray(src)
+    if a.ndim == 2:
+        a = a[None]
+    cplx = np.iscomplexobj(a)
+    a = np.ascontiguousarray(a, dtype=np.complex128 if cplx else np.float64)
+    Np, Ny, Nx = a.shape
+    pos = _f32(pos)
+    M = pos.shape[0]
+    out = np.empty((M, Np, T, T), dtype=a.dtype)
+    _check(_load().oracle_extract_tiles(_p64(a), 2 if cplx else 1, Nx, Ny, Np, _p32(pos), M, _sf(dx), int(T), _p64(out)),
+           "oracle_extract_tiles")
+    return out
+
+
+def lightsheet(Nx, Ny, dx, lam, n0, NA, z_focus) -> np.ndarray:
+    out = np.empty((Ny, Nx), dtype=np.complex128)
+    _check(_load().oracle_lightsheet(Nx, Ny, _sf(dx), _sf(lam), _sf(n0), _sf(NA), _sf(z_focus), _p64(out)),
+           "oracle_lightsheet")
+    return out
+
+
+def multiplex_annular(pos, phase, amp, NA_in, NA_out, Nx, Ny, dx, lam) -> np.ndarray:
+    pos = _f32(pos)
+    M = pos.shape[0]
+    phase = _f32(phase, (M,))
+    amp = _f32(amp, (M,))
+    out = np.empty((Ny, Nx), dtype=np.complex128)
+    _check(_load().oracle_multiplex_annular(_p32(pos), _p32(phase), _p32(amp), M, _sf(NA_in), _sf(NA_out),
+                                            Nx, Ny, _sf(dx), _sf(lam), _p64(out)), "oracle_multiplex_annular")
+    return out
+
+
+def image_formation(S, pos, dx, psf) -> np.ndarray:
+    """Camera image of one object plane with a piecewise-constant spatially varying PSF
+    (``oracle_image_formation``): S [Ny][Nx], psf [M][T][T]."""
+    S = np.ascontiguousarray(S, dtype=np.float64)
+    psf = np.ascontiguousarray(psf, dtype=np.float64)
+    Ny, Nx = S.shape
+    pos = _f32(pos)
+    M, T = psf.shape[0], psf.shape[1]
+    out = np.empty((Ny, Nx), dtype=np.float64)
+    _check(_load().oracle_image_formation(_p64(S), Nx, Ny, _p32(pos), M, _sf(dx), _p64(psf), T, _p64(out)),
+           "oracle_image_formation")
     return out
