@@ -21,8 +21,10 @@
  * Conventions.  All lengths in micrometres; lambda is the vacuum wavelength.  Arrays are
  * row-major with x fastest: field [B][Ny][Nx] of float pairs (re, im) = complex64,
  * volumes [Nz][Ny][Nx] float32.  Scalars are float32; every table is built in double from
- * the float32 values promoted to double.  Nx and Ny must be powers of two in [32, 1024]
- * (Nx != Ny allowed).  Periodic lateral boundaries (plain FFT).
+ * the float32 values promoted to double.  Nx and Ny must be powers of two in [32, 2048]
+ * (Nx != Ny allowed; SURVEY 8b asks for [128, 2048], PAPER.md line 31 uses 1024 x 2048); a grid
+ * with a 2048-point side needs both sides >= 256, and bb_fft2 / bb_multiplex_* stop at 1024.
+ * Periodic lateral boundaries (plain FFT).
  *
  * Pointers.  Unless a parameter says HOST, pointers are DEVICE pointers on the current CUDA
  * device (e.g. torch tensor data_ptr()).  The caller owns every buffer in a signature; the
@@ -50,7 +52,7 @@ extern "C" {
 typedef enum {
     BB_OK = 0,
     BB_ERR_INVALID_ARG = 1,        /* NULL pointer, non-positive scalar, bad count, bad flags */
-    BB_ERR_UNSUPPORTED_SHAPE = 2,  /* Nx or Ny not a power of two in [32, 1024] */
+    BB_ERR_UNSUPPORTED_SHAPE = 2,  /* Nx or Ny not a power of two in the supported range (see above) */
     BB_ERR_CUDA = 3,               /* a CUDA call failed (message in bb_last_error) */
     BB_ERR_OOM = 4,                /* device or host allocation failed */
     BB_ERR_ARCH = 5,               /* current device is not compute capability 10.x */
@@ -62,14 +64,25 @@ typedef enum {
 #define BB_INTENSITY_PER_FIELD 2u  /* intensity_out is [B][Nz][Ny][Nx], not summed over the batch */
 #define BB_LAUNCH_PER_PHASE    4u  /* diagnostic: one kernel launch per half-step instead of one
                                       persistent cooperative kernel (same arithmetic, same results) */
+#define BB_BACKWARD            8u  /* time-reversed (phase-conjugate) propagation, PAPER.md line 27 (Fig. 2c: "reversal
+                                      of guide star emitted light fields") and line 33: for j = Nz-1 .. 0
+                                          I[j] = |u|^2;  u *= conj(screen_j);  U = FFT2(u);  U *= conj(H_j);  u = IFFT2(U)
+                                      (evanescent modes stay cut).  field in: u at z = Nz dz; out: u at z = 0.
+                                      Undoes a forward run exactly where no mode is evanescent. */
+#define BB_HOMOGENEOUS        16u  /* no sample: Nz steps through the medium n0 (no phase screen; dn_volume is not
+                                      read and may be NULL; nref must be NULL).  intensity_out[j] = |u|^2 after step j:
+                                      the through-focus stack of a field ("volumetric PSFs") */
 
 typedef struct {
     int struct_size;     /* sizeof(bb_opts); lets the struct grow compatibly */
     int batch;           /* B >= 1 independent fields, contiguous [B][Ny][Nx], one shared dn volume
                             (north_star item 4, BASELINE.json configs[4]) */
     const float *nref;   /* HOST float[Nz]: reference index n_ref[j] of step j (reading A3),
-                            or NULL = n0 for every step */
-    unsigned flags;      /* BB_ACCUMULATE | BB_INTENSITY_PER_FIELD | BB_LAUNCH_PER_PHASE */
+                            or NULL = n0 for every step.  HOST, not device (a deviation from SURVEY 8b):
+                            the host picks the cached propagator table of every step and the live
+                            kx band from n_ref before it enqueues anything; a device array would have
+                            to be copied back and waited for at that point. */
+    unsigned flags;      /* BB_ACCUMULATE | BB_INTENSITY_PER_FIELD | BB_LAUNCH_PER_PHASE | BB_BACKWARD | BB_HOMOGENEOUS */
     void *stream;        /* cudaStream_t; NULL = the legacy default stream */
 } bb_opts;
 
@@ -83,7 +96,13 @@ typedef struct {
 int bb_propagate(void *field, const float *dn_volume, int Nx, int Ny, int Nz,
                  float dx, float dz, float lambda, float n0, float *intensity_out);
 
-/* Same with options (batch, adapted n_ref, accumulate / per-field intensity, stream). opts may be NULL. */
+/* Same with options (batch, adapted n_ref, accumulate / per-field intensity, backward, homogeneous,
+ * stream).  opts may be NULL.  Kernel selection (results do not depend on it beyond rounding): grids
+ * with sides in {256, 512, 1024} run the 16-point-thread kernel -- for a batch only while the screen
+ * factors of a CTA's rows fit its buffer, ceil(Ny / SMs) * Nx <= 8192 -- sides of 2048 the
+ * 8-point-thread kernel, everything else the 32-point-thread kernel.  The summed intensity of a
+ * batch is accumulated with shared-memory atomics: its summation order, hence its last bits, can
+ * differ between runs (tolerance contract: relative L2 <= 1e-4 against the definition). */
 int bb_propagate_ex(void *field, const float *dn_volume, int Nx, int Ny, int Nz,
                     float dx, float dz, float lambda, float n0, float *intensity_out,
                     const bb_opts *opts);
@@ -125,6 +144,57 @@ int bb_nref_from_dn(const float *dn_volume, int Nx, int Ny, int Nz, float n0, in
 int bb_multiplex_psf(const float *emitter_positions, const float *emitter_phase,
                      const float *emitter_amp, int M, float NA,
                      int Nx, int Ny, float dx, float lambda, void *field_out, void *stream);
+
+/*
+ * bb_multiplex_annular -- the same with an annular pupil NA_inner <= |k| / k0 <= NA: every "emitter"
+ * is a Bessel-beam focus (a thin annulus gives J0(k0 NA r)), a row of them a Bessel lattice
+ * ("Bessel lattices"; line 17, Fig. 1d).  NA_inner = 0 is bb_multiplex_psf.
+ */
+int bb_multiplex_annular(const float *emitter_positions, const float *emitter_phase,
+                         const float *emitter_amp, int M, float NA_inner, float NA,
+                         int Nx, int Ny, float dx, float lambda, void *field_out, void *stream);
+
+/*
+ * bb_lightsheet -- PAPER.md line 29 ("a cylindrical sheet of light is propagated"), BASELINE.json
+ * configs[1] ("cylindrically focused Gaussian sheet (NA 0.1 in y, flat in x)"): the input-plane field of
+ * a sheet whose waist exp(-y^2 / w0^2), w0 = lambda / (pi NA), lies z_focus behind the input plane in
+ * the medium n0 -- the waist propagated back by z_focus with the exact propagator (evanescent ky
+ * cut), uniform in x, y_i = (i - Ny/2) dx.  field_out: float pairs [Ny][Nx].
+ */
+int bb_lightsheet(int Nx, int Ny, float dx, float lambda, float n0, float NA, float z_focus,
+                  void *field_out, void *stream);
+
+/*
+ * bb_refocus -- PAPER.md lines 29-31 ("propagating light from multiplexed diffraction-limited
+ * point-sources orthogonally through an idealized, refocusing lens towards the camera"): free-space
+ * propagation of `batch` fields over the SIGNED distance dz in a homogeneous medium of index n,
+ *     U = FFT2(u);  U *= (s > 0) ? exp(i dz sqrt(s)) : 0;  u = IFFT2(U),   s = (k0 n)^2 - kx^2 - ky^2
+ * in place (dz < 0 refocuses the exit field of a sample onto the emitter plane; dz = 0 only cuts the
+ * evanescent modes).  A through-focus stack is bb_propagate_ex with BB_HOMOGENEOUS.
+ */
+int bb_refocus(void *field, int Nx, int Ny, int batch, float dx, float dz, float lambda, float n, void *stream);
+
+/*
+ * bb_extract_tiles -- PAPER.md line 31 ("quasi-continuum of spatially-dependent, volumetric PSFs"): the
+ * T x T window around every emitter in every plane of a stack.  src: [Nplanes][Ny][Nx] of `elem` floats
+ * per pixel (1: intensity, 2: complex field); emitter e has centre pixel (floor(x_e / dx + 0.5) + Nx/2,
+ * floor(y_e / dx + 0.5) + Ny/2) (coordinates as in bb_multiplex_psf) and window [c - T/2, c - T/2 + T) per
+ * axis, periodic.  tiles_out: [M][Nplanes][T][T] of `elem` floats.
+ */
+int bb_extract_tiles(const void *src, int elem, int Nx, int Ny, int Nplanes, const float *emitter_positions,
+                     int M, float dx, int T, void *tiles_out, void *stream);
+
+/*
+ * bb_image_formation -- PAPER.md line 31 ("Convolving the exhaustively sampled set of spatially-varying PSFs
+ * with the fluorescent object"; line 17, Fig. 1c), reading A18: the PSF is piecewise constant over
+ * the cells of the emitter grid.  source S = fluorophore density x excitation intensity, float [Ny][Nx]; a source
+ * pixel r' radiates with the intensity tile of the emitter nearest to it (periodic distance, lowest index on ties):
+ *     image[r] = sum_{r'} S[r'] psf[e(r')][r - r' + T/2]        (r' over the T x T neighbourhood, periodic)
+ * psf_tiles: float [M][T][T] (e.g. from bb_extract_tiles, T <= 96), image_out: float [Ny][Nx].  Uses the
+ * library's workspace: calls on one device must not overlap.
+ */
+int bb_image_formation(const float *source, int Nx, int Ny, const float *emitter_positions, int M, float dx,
+                       const float *psf_tiles, int T, float *image_out, void *stream);
 
 /*
  * Building blocks, exported so that each can be checked against the oracle on its own.

@@ -18,10 +18,13 @@ LIB_PATH = os.path.join(_HERE, "libbiobeam_b200.so")
 ACCUMULATE = 1
 INTENSITY_PER_FIELD = 2
 LAUNCH_PER_PHASE = 4
+BACKWARD = 8
+HOMOGENEOUS = 16
 
 EXPORTS = ("bb_propagate", "bb_propagate_ex", "bb_propagate_host", "bb_nref_from_dn",
            "bb_multiplex_psf", "bb_fft2", "bb_propagator_table", "bb_last_error", "bb_version",
-           "bb_shutdown", "bb_launch_count", "bb_device_status", "bb_probe_l2_bandwidth", "bb_probe_fp32", "bb_probe_trace")
+           "bb_shutdown", "bb_launch_count", "bb_device_status", "bb_probe_l2_bandwidth", "bb_probe_fp32", "bb_probe_trace",
+           "bb_multiplex_annular", "bb_lightsheet", "bb_refocus", "bb_extract_tiles", "bb_image_formation")
 
 STATUS_NAMES = {0: "BB_OK", 1: "BB_ERR_INVALID_ARG", 2: "BB_ERR_UNSUPPORTED_SHAPE", 3: "BB_ERR_CUDA",
                 4: "BB_ERR_OOM", 5: "BB_ERR_ARCH", 6: "BB_ERR_INTERNAL"}
@@ -58,6 +61,11 @@ def load() -> ctypes.CDLL:
     lib.bb_propagate_host.argtypes = [vp, vp, i, i, i, f, f, f, f, vp, ctypes.POINTER(_Opts)]
     lib.bb_nref_from_dn.argtypes = [vp, i, i, i, f, i, fp, vp]
     lib.bb_multiplex_psf.argtypes = [vp, vp, vp, i, f, i, i, f, f, vp, vp]
+    lib.bb_multiplex_annular.argtypes = [vp, vp, vp, i, f, f, i, i, f, f, vp, vp]
+    lib.bb_lightsheet.argtypes = [i, i, f, f, f, f, f, vp, vp]
+    lib.bb_refocus.argtypes = [vp, i, i, i, f, f, f, f, vp]
+    lib.bb_extract_tiles.argtypes = [vp, i, i, i, i, vp, i, f, i, vp, vp]
+    lib.bb_image_formation.argtypes = [vp, i, i, vp, i, f, vp, i, vp, vp]
     lib.bb_fft2.argtypes = [vp, i, i, i, i, vp]
     lib.bb_propagator_table.argtypes = [i, i, f, f, f, f, vp, vp]
     lib.bb_probe_l2_bandwidth.argtypes = [ctypes.c_ulonglong, i, i, ctypes.POINTER(ctypes.c_double)]
@@ -98,18 +106,23 @@ def _f32(t: torch.Tensor, name: str):
 
 
 def propagate(field: torch.Tensor, dn: torch.Tensor, dx: float, dz: float, lam: float, n0: float,
-              intensity: Optional[torch.Tensor] = None, nref=None, flags: int = 0, stream=None):
+              intensity: Optional[torch.Tensor] = None, nref=None, flags: int = 0, stream=None, nz=None):
     """``bb_propagate_ex`` (CUDA tensors; asynchronous on ``stream``) or ``bb_propagate_host``
     (CPU tensors, pinned for overlap; synchronous).  ``field`` is updated in place.
     ``nref``: None or a sequence / CPU tensor of Nz floats."""
     lib = load()
     B, Ny, Nx = _field_shape(field)
-    _f32(dn, "dn")
-    if dn.dim() != 3 or dn.shape[1] != Ny or dn.shape[2] != Nx:
-        raise TypeError("dn must be [Nz][%d][%d]" % (Ny, Nx))
-    Nz = dn.shape[0]
     on_gpu = field.is_cuda
-    if dn.is_cuda != on_gpu or (intensity is not None and intensity.is_cuda != on_gpu):
+    if dn is None:
+        if not flags & HOMOGENEOUS or nz is None:
+            raise TypeError("dn may be None only with HOMOGENEOUS and nz = number of steps")
+        Nz = int(nz)
+    else:
+        _f32(dn, "dn")
+        if dn.dim() != 3 or dn.shape[1] != Ny or dn.shape[2] != Nx:
+            raise TypeError("dn must be [Nz][%d][%d]" % (Ny, Nx))
+        Nz = dn.shape[0]
+    if (dn is not None and dn.is_cuda != on_gpu) or (intensity is not None and intensity.is_cuda != on_gpu):
         raise TypeError("field, dn and intensity must all be CUDA tensors or all CPU tensors")
     if intensity is not None:
         _f32(intensity, "intensity")
@@ -125,13 +138,14 @@ def propagate(field: torch.Tensor, dn: torch.Tensor, dx: float, dz: float, lam: 
         nref_buf = (ctypes.c_float * Nz)(*[float(x) for x in nref])
         opts.nref = ctypes.cast(nref_buf, ctypes.POINTER(ctypes.c_float))
     iptr = ctypes.c_void_p(intensity.data_ptr()) if intensity is not None else None
+    dnp = ctypes.c_void_p(dn.data_ptr()) if dn is not None else None
     if on_gpu:
         opts.stream = _stream_ptr(stream)
         with torch.cuda.device(field.device):
-            rc = lib.bb_propagate_ex(ctypes.c_void_p(field.data_ptr()), ctypes.c_void_p(dn.data_ptr()), Nx, Ny, Nz,
+            rc = lib.bb_propagate_ex(ctypes.c_void_p(field.data_ptr()), dnp, Nx, Ny, Nz,
                                      dx, dz, lam, n0, iptr, ctypes.byref(opts))
     else:
-        rc = lib.bb_propagate_host(ctypes.c_void_p(field.data_ptr()), ctypes.c_void_p(dn.data_ptr()), Nx, Ny, Nz,
+        rc = lib.bb_propagate_host(ctypes.c_void_p(field.data_ptr()), dnp, Nx, Ny, Nz,
                                    dx, dz, lam, n0, iptr, ctypes.byref(opts))
     _check(rc)
     return field, intensity
@@ -177,6 +191,67 @@ def multiplex_psf(pos: torch.Tensor, phase: Optional[torch.Tensor], amp: Optiona
     p = lambda t: ctypes.c_void_p(t.data_ptr()) if t is not None else None
     with torch.cuda.device(pos.device):
         _check(lib.bb_multiplex_psf(p(pos), p(phase), p(amp), M, NA, Nx, Ny, dx, lam, p(out), _stream_ptr(stream)))
+    return out
+
+
+def multiplex_annular(pos: torch.Tensor, phase: Optional[torch.Tensor], amp: Optional[torch.Tensor], NA_in: float, NA: float,
+                      Nx: int, Ny: int, dx: float, lam: float, out: Optional[torch.Tensor] = None, stream=None):
+    """``bb_multiplex_annular``: Bessel-beam foci / lattices (annular pupil NA_in <= |k|/k0 <= NA)."""
+    lib = load()
+    _f32(pos, "pos")
+    M = pos.shape[0]
+    if out is None:
+        out = torch.empty((Ny, Nx), dtype=torch.complex64, device=pos.device)
+    p = lambda t: ctypes.c_void_p(t.data_ptr()) if t is not None else None
+    with torch.cuda.device(pos.device):
+        _check(lib.bb_multiplex_annular(p(pos), p(phase), p(amp), M, NA_in, NA, Nx, Ny, dx, lam, p(out), _stream_ptr(stream)))
+    return out
+
+
+def lightsheet(Nx: int, Ny: int, dx: float, lam: float, n0: float, NA: float, z_focus: float, device="cuda", stream=None):
+    """``bb_lightsheet``: input-plane field of a cylindrical Gaussian sheet focused z_focus behind the plane."""
+    out = torch.empty((Ny, Nx), dtype=torch.complex64, device=device)
+    with torch.cuda.device(out.device):
+        _check(load().bb_lightsheet(Nx, Ny, dx, lam, n0, NA, z_focus, ctypes.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+    return out
+
+
+def refocus(field: torch.Tensor, dx: float, dz: float, lam: float, n: float, stream=None) -> torch.Tensor:
+    """``bb_refocus``: in-place free-space propagation over the signed distance dz in index n."""
+    B, Ny, Nx = _field_shape(field)
+    with torch.cuda.device(field.device):
+        _check(load().bb_refocus(ctypes.c_void_p(field.data_ptr()), Nx, Ny, B, dx, dz, lam, n, _stream_ptr(stream)))
+    return field
+
+
+def extract_tiles(src: torch.Tensor, pos: torch.Tensor, dx: float, T: int, stream=None) -> torch.Tensor:
+    """``bb_extract_tiles``: src [Np][Ny][Nx] (or [Ny][Nx]), float32 or complex64 -> [M][Np][T][T]."""
+    if src.dim() == 2:
+        src = src[None]
+    if src.dtype not in (torch.float32, torch.complex64) or not src.is_contiguous() or src.dim() != 3:
+        raise TypeError("src must be a contiguous float32 or complex64 tensor [Np][Ny][Nx]")
+    _f32(pos, "pos")
+    Np, Ny, Nx = src.shape
+    M = pos.shape[0]
+    out = torch.empty((M, Np, T, T), dtype=src.dtype, device=src.device)
+    with torch.cuda.device(src.device):
+        _check(load().bb_extract_tiles(ctypes.c_void_p(src.data_ptr()), 2 if src.dtype == torch.complex64 else 1, Nx, Ny, Np,
+                                       ctypes.c_void_p(pos.data_ptr()), M, dx, T, ctypes.c_void_p(out.data_ptr()),
+                                       _stream_ptr(stream)))
+    return out
+
+
+def image_formation(source: torch.Tensor, pos: torch.Tensor, dx: float, psf: torch.Tensor, stream=None) -> torch.Tensor:
+    """``bb_image_formation``: source [Ny][Nx] float32, psf [M][T][T] float32 -> image [Ny][Nx]."""
+    _f32(source, "source"); _f32(pos, "pos"); _f32(psf, "psf")
+    Ny, Nx = source.shape
+    M, T = psf.shape[0], psf.shape[1]
+    if pos.shape[0] != M or psf.shape[2] != T:
+        raise TypeError("psf must be [M][T][T] with M = number of emitters")
+    out = torch.empty_like(source)
+    with torch.cuda.device(source.device):
+        _check(load().bb_image_formation(ctypes.c_void_p(source.data_ptr()), Nx, Ny, ctypes.c_void_p(pos.data_ptr()), M, dx,
+                                         ctypes.c_void_p(psf.data_ptr()), T, ctypes.c_void_p(out.data_ptr()), _stream_ptr(stream)))
     return out
 
 

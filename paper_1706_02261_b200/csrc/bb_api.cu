@@ -25,6 +25,7 @@ std::mutex g_mu;
 unsigned long long g_launches = 0;
 long long *g_trace = nullptr;      // bb_probe_trace
 int g_trace_phases = 0;
+int g_trace_dev = -1;
 
 int fail(int code, const char *fmt, ...) {
     char buf[512];
@@ -89,7 +90,19 @@ struct Plan {
 
 std::vector<Plan *> g_plans;
 struct Workspace { void *ptr = nullptr; size_t bytes = 0; };
-Workspace g_ws_field, g_ws_dn, g_ws_I, g_ws_misc;
+// Everything the library allocates outside a plan belongs to ONE device: workspaces of the host-buffer
+// entry point and of the helpers, its copy / compute streams and their events (created once, reused).
+struct DeviceCtx {
+    Workspace field, dn, I, misc;
+    cudaStream_t s_in = nullptr, s_run = nullptr, s_out = nullptr;
+    std::vector<cudaEvent_t> events;
+};
+std::map<int, DeviceCtx> g_ctx;
+DeviceCtx &device_ctx() {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    return g_ctx[dev];
+}
 
 int check_arch(int *device_out, int *sm_count) {
     int dev = 0;
@@ -303,7 +316,8 @@ bool shape_ok(int Nx, int Ny) {
 int validate_common(const void *field, const float *dn, int Nx, int Ny, int Nz, float dx, float dz,
                     float lambda, float n0, const bb_opts *opts, int *B, unsigned *flags) {
     if (!field) return fail(BB_ERR_INVALID_ARG, "field is NULL");
-    if (!dn) return fail(BB_ERR_INVALID_ARG, "dn_volume is NULL");
+    const bool homogeneous = opts && (opts->flags & BB_HOMOGENEOUS);
+    if (!dn && !homogeneous) return fail(BB_ERR_INVALID_ARG, "dn_volume is NULL (only BB_HOMOGENEOUS runs without one)");
     if (Nz < 1) return fail(BB_ERR_INVALID_ARG, "Nz = %d must be >= 1", Nz);
     if (!(dx > 0.f) || !(dz > 0.f) || !(lambda > 0.f) || !(n0 > 0.f) || !std::isfinite(dx) ||
         !std::isfinite(dz) || !std::isfinite(lambda) || !std::isfinite(n0))
@@ -316,8 +330,10 @@ int validate_common(const void *field, const float *dn, int Nx, int Ny, int Nz, 
         if (opts->struct_size != (int)sizeof(bb_opts))
             return fail(BB_ERR_INVALID_ARG, "bb_opts.struct_size = %d, expected %d", opts->struct_size, (int)sizeof(bb_opts));
         if (opts->batch < 1) return fail(BB_ERR_INVALID_ARG, "batch = %d must be >= 1", opts->batch);
-        if (opts->flags & ~(BB_ACCUMULATE | BB_INTENSITY_PER_FIELD | BB_LAUNCH_PER_PHASE))
+        if (opts->flags & ~(BB_ACCUMULATE | BB_INTENSITY_PER_FIELD | BB_LAUNCH_PER_PHASE | BB_BACKWARD | BB_HOMOGENEOUS))
             return fail(BB_ERR_INVALID_ARG, "unknown flag bits 0x%x", opts->flags);
+        if (homogeneous && opts->nref)
+            return fail(BB_ERR_INVALID_ARG, "BB_HOMOGENEOUS propagates in the medium n0: nref must be NULL");
         if (opts->nref)
             for (int j = 0; j < Nz; ++j)
                 if (!(opts->nref[j] > 0.f) || !std::isfinite(opts->nref[j]))
@@ -399,16 +415,21 @@ int launch_steps(Plan *p, cf *field, const float *dn, float *inten, long long in
     P.tw256 = p->tw256; P.twcx = p->twcx; P.twcy = p->twcy;
     P.fmax = p->d_fmax; P.cw4 = p->cw4;
     P.flags = flags & 3u;
+    P.backward = (flags & BB_BACKWARD) ? 1 : 0;
+    P.noscreen = (flags & BB_HOMOGENEOUS) ? 1 : 0;
     const bool k8 = use_k8(p, B), k16 = use_k16(p, B);
     if (!k8 && !k16 && !p->k32) return fail(BB_ERR_UNSUPPORTED_SHAPE, "no kernel for Nx = %d, Ny = %d, batch = %d", p->Nx, p->Ny, B);
     if (k16 || k8) P.use_tma = make_field_tmap(&P.tmap, field, p->Nx, p->Ny, B, p->cw4 ? 4 : 8) ? 1 : 0;
-    if (g_trace && (k16 || k8) && 2 * j1 + 1 <= g_trace_phases) { P.trace = g_trace; P.trace_p0 = 0; }
+    if (g_trace && g_trace_dev == p->device && (k16 || k8) && 2 * Nz_total + 1 <= g_trace_phases) { P.trace = g_trace; P.trace_p0 = 0; }
     auto launch = [&](bool coop) {
         return k8 ? bb::kernel8_launch(p->Nx, p->Ny, P, p->grid, coop, s)
                   : k16 ? bb::kernel16_launch(p->Nx, p->Ny, P, p->grid, coop, s)
                         : bb::kernel_launch(p->Nx, p->Ny, P, p->grid, coop, s);
     };
+    // steps [j0, j1): forward = column phases j0 .. j1-1 and the row phases after them (plus row phase 0);
+    // backward = row / column phases Nz-j1 .. Nz-1-j0 in that order (plus the closing row phase Nz)
     int p0 = (j0 == 0) ? 0 : 2 * j0 + 1, p1 = 2 * j1 + 1;
+    if (flags & BB_BACKWARD) { p0 = 2 * (Nz_total - j1); p1 = 2 * (Nz_total - j0) + (j0 == 0 ? 1 : 0); }
     if (flags & BB_LAUNCH_PER_PHASE) {
         for (int ph = p0; ph < p1; ++ph) {
             P.p0 = ph; P.p1 = ph + 1;
@@ -426,20 +447,26 @@ int launch_steps(Plan *p, cf *field, const float *dn, float *inten, long long in
     return BB_OK;
 }
 
-// Per-step tables and phase offsets for steps [j0, *j_done): the longest prefix of [j0, Nz)
-// whose distinct propagator tables fit the cache together (normally all of it).
-int prepare_steps(Plan *p, int B, int Nz, int j0, float dx, float dz, float lambda, float n0, const float *nref,
-                  cudaStream_t s, std::vector<const cf *> &h_tab, std::vector<float> &h_phase, int *j_done) {
+// Per-step tables and phase offsets for the steps at positions [i0, *i_done) of the processing order
+// (forward: step j = i; backward: j = Nz - 1 - i): the longest run whose distinct propagator tables
+// fit the cache together (normally all of it).  Backward steps use the conjugate factors, i.e. the
+// table and the phase offset of -dz.
+int prepare_steps(Plan *p, int B, int Nz, int i0, float dx, float dz, float lambda, float n0, const float *nref,
+                  unsigned flags, cudaStream_t s, std::vector<const cf *> &h_tab, std::vector<float> &h_phase, int *i_done) {
     std::vector<int> h_fmax(Nz);
+    const bool backward = (flags & BB_BACKWARD) != 0;
+    const float dzs = backward ? -dz : dz;
     double k0 = kTwoPi / (double)lambda;
     unsigned long long protect = ++p->tick;
     const cf *last_ptr = nullptr;
     float last_nref = 0.f;
-    int j = j0;
-    for (; j < Nz; ++j) {
+    const bool noprune = getenv("BB_K16_NOPRUNE") != nullptr;
+    int i = i0;
+    for (; i < Nz; ++i) {
+        const int j = backward ? Nz - 1 - i : i;
         float nr = nref ? nref[j] : n0;
         if (!(last_ptr && nr == last_nref)) {
-            TableKey key = {dx, dz, lambda, nr, (use_k16(p, B) || use_k8(p, B)) ? p->Nx / 256 : 1};
+            TableKey key = {dx, dzs, lambda, nr, (use_k16(p, B) || use_k8(p, B)) ? p->Nx / 256 : 1};
             cf *ptr = nullptr;
             int rc = get_table(p, key, s, protect, &ptr);
             if (rc == kTableCacheFull) break;                 // the rest goes into the next launch
@@ -447,19 +474,17 @@ int prepare_steps(Plan *p, int B, int Nz, int j0, float dx, float dz, float lamb
             last_ptr = ptr; last_nref = nr;
         }
         h_tab[j] = last_ptr;
-        h_phase[j] = (float)(k0 * (double)dz * ((double)n0 - (double)nr));
-        h_fmax[j] = getenv("BB_K16_NOPRUNE") ? p->Nx / 2 : live_fmax(p->Nx, (double)dx, k0 * (double)nr);
+        h_phase[j] = (float)(k0 * (double)dzs * ((double)n0 - (double)nr));
+        h_fmax[j] = noprune ? p->Nx / 2 : live_fmax(p->Nx, (double)dx, k0 * (double)nr);
     }
-    *j_done = j;
-    if (j == j0) return BB_OK;
+    *i_done = i;
+    if (i == i0) return BB_OK;
     int rc = ensure_steps(p, Nz);
     if (rc) return rc;
-    BB_CUDA(cudaMemcpyAsync((void *)(p->d_htab + j0), h_tab.data() + j0, (size_t)(j - j0) * sizeof(cf *),
-                            cudaMemcpyHostToDevice, s));
-    BB_CUDA(cudaMemcpyAsync(p->d_phase + j0, h_phase.data() + j0, (size_t)(j - j0) * sizeof(float),
-                            cudaMemcpyHostToDevice, s));
-    BB_CUDA(cudaMemcpyAsync(p->d_fmax + j0, h_fmax.data() + j0, (size_t)(j - j0) * sizeof(int),
-                            cudaMemcpyHostToDevice, s));
+    const int ja = backward ? Nz - i : i0, n = i - i0;         // the steps touched are the range [ja, ja + n)
+    BB_CUDA(cudaMemcpyAsync((void *)(p->d_htab + ja), h_tab.data() + ja, (size_t)n * sizeof(cf *), cudaMemcpyHostToDevice, s));
+    BB_CUDA(cudaMemcpyAsync(p->d_phase + ja, h_phase.data() + ja, (size_t)n * sizeof(float), cudaMemcpyHostToDevice, s));
+    BB_CUDA(cudaMemcpyAsync(p->d_fmax + ja, h_fmax.data() + ja, (size_t)n * sizeof(int), cudaMemcpyHostToDevice, s));
     return BB_OK;
 }
 
@@ -605,13 +630,24 @@ void bb_shutdown(void) {
         for (TableEntry &e : p->tables) cudaFree(e.ptr);
         if (p->d_htab) cudaFree((void *)p->d_htab);
         if (p->d_phase) cudaFree(p->d_phase);
+        if (p->d_fmax) cudaFree(p->d_fmax);
         delete p;
     }
     g_plans.clear();
-    for (Workspace *w : {&g_ws_field, &g_ws_dn, &g_ws_I, &g_ws_misc}) {
-        if (w->ptr) cudaFree(w->ptr);
-        w->ptr = nullptr; w->bytes = 0;
+    for (auto &kv : g_ctx) {
+        DeviceCtx &c = kv.second;
+        for (Workspace *w : {&c.field, &c.dn, &c.I, &c.misc}) {
+            if (w->ptr) cudaFree(w->ptr);
+            w->ptr = nullptr; w->bytes = 0;
+        }
+        for (cudaEvent_t e : c.events) cudaEventDestroy(e);
+        c.events.clear();
+        for (cudaStream_t *st : {&c.s_in, &c.s_run, &c.s_out}) {
+            if (*st) cudaStreamDestroy(*st);
+            *st = nullptr;
+        }
     }
+    g_ctx.clear();
 }
 
 int bb_device_status(void) {
@@ -629,11 +665,13 @@ int bb_device_status(void) {
     return BB_OK;
 }
 
-int bb_propagate_ex(void *field, const float *dn, int Nx, int Ny, int Nz, float dx, float dz, float lambda,
-                    float n0, float *intensity_out, const bb_opts *opts) {
-    std::lock_guard<std::mutex> lk(g_mu);
+}  // extern "C"
+namespace {
+// bb_propagate_ex without the lock (the helpers that are propagations in disguise call it too)
+int propagate_impl(void *field, const float *dn, int Nx, int Ny, int Nz, float dx, float dz, float lambda,
+                   float n0, float *intensity_out, const bb_opts *opts, bool allow_zero_dz = false) {
     int B; unsigned flags;
-    int rc = validate_common(field, dn, Nx, Ny, Nz, dx, dz, lambda, n0, opts, &B, &flags);
+    int rc = validate_common(field, dn, Nx, Ny, Nz, dx, allow_zero_dz && dz == 0.f ? 1.f : dz, lambda, n0, opts, &B, &flags);
     if (rc) return rc;
     Plan *p;
     rc = get_plan(Nx, Ny, &p);
@@ -644,26 +682,120 @@ int bb_propagate_ex(void *field, const float *dn, int Nx, int Ny, int Nz, float 
     std::vector<const cf *> h_tab(Nz);
     std::vector<float> h_phase(Nz);
     double k0 = kTwoPi / (double)lambda;
-    float phase_b = (float)(k0 * (double)dz);
+    const bool backward = (flags & BB_BACKWARD) != 0;
+    float phase_b = (float)(k0 * (double)(backward ? -dz : dz));
     size_t npx = (size_t)Nx * Ny;
-    int j0 = 0;
-    while (j0 < Nz) {
-        int j1;
-        rc = prepare_steps(p, B, Nz, j0, dx, dz, lambda, n0, nref, s, h_tab, h_phase, &j1);
+    int i0 = 0;                                               // position in the processing order
+    while (i0 < Nz) {
+        int i1;
+        rc = prepare_steps(p, B, Nz, i0, dx, dz, lambda, n0, nref, flags, s, h_tab, h_phase, &i1);
         if (rc) return rc;
-        if (j1 <= j0) return fail(BB_ERR_OOM, "propagator table cache too small for one step");
-        rc = launch_steps(p, (cf *)field, dn + (size_t)j0 * npx,
+        if (i1 <= i0) return fail(BB_ERR_OOM, "propagator table cache too small for one step");
+        const int j0 = backward ? Nz - i1 : i0, j1 = backward ? Nz - i0 : i1;   // the steps of this launch
+        rc = launch_steps(p, (cf *)field, dn ? dn + (size_t)j0 * npx : nullptr,
                           intensity_out ? intensity_out + (size_t)j0 * npx : nullptr,
                           (long long)Nz * (long long)npx, B, Nz, j0, j1, phase_b, flags, s);
         if (rc) return rc;
-        j0 = j1;
+        i0 = i1;
     }
     return BB_OK;
+}
+}  // namespace
+extern "C" {
+
+int bb_propagate_ex(void *field, const float *dn, int Nx, int Ny, int Nz, float dx, float dz, float lambda,
+                    float n0, float *intensity_out, const bb_opts *opts) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    return propagate_impl(field, dn, Nx, Ny, Nz, dx, dz, lambda, n0, intensity_out, opts);
+}
+
+int bb_refocus(void *field, int Nx, int Ny, int batch, float dx, float dz, float lambda, float n, void *stream) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!std::isfinite(dz)) return fail(BB_ERR_INVALID_ARG, "dz must be finite");
+    bb_opts o;
+    o.struct_size = (int)sizeof(bb_opts);
+    o.batch = batch;
+    o.nref = nullptr;
+    o.flags = BB_HOMOGENEOUS | (dz < 0.f ? BB_BACKWARD : 0u);      // conj(H(|dz|)) = H(-|dz|), evanescent modes cut either way
+    o.stream = stream;
+    return propagate_impl(field, nullptr, Nx, Ny, 1, dx, std::fabs(dz), lambda, n, nullptr, &o, true);
 }
 
 int bb_propagate(void *field, const float *dn, int Nx, int Ny, int Nz, float dx, float dz, float lambda,
                  float n0, float *intensity_out) {
     return bb_propagate_ex(field, dn, Nx, Ny, Nz, dx, dz, lambda, n0, intensity_out, nullptr);
+}
+
+int bb_extract_tiles(const void *src, int elem, int Nx, int Ny, int Nplanes, const float *emitter_positions, int M,
+                     float dx, int T, void *tiles_out, void *stream) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!src || !emitter_positions || !tiles_out) return fail(BB_ERR_INVALID_ARG, "src, emitter_positions or tiles_out is NULL");
+    if (elem != 1 && elem != 2) return fail(BB_ERR_INVALID_ARG, "elem = %d must be 1 (float) or 2 (float pairs)", elem);
+    if (Nx < 1 || Ny < 1 || Nplanes < 1 || M < 1 || M > 65535 || Nplanes > 65535)
+        return fail(BB_ERR_INVALID_ARG, "Nx, Ny, Nplanes, M must be >= 1 (Nplanes, M <= 65535)");
+    if (T < 1 || T > Nx || T > Ny) return fail(BB_ERR_INVALID_ARG, "tile size T = %d must be in [1, min(Nx, Ny)]", T);
+    if (!(dx > 0.f) || !std::isfinite(dx)) return fail(BB_ERR_INVALID_ARG, "dx must be positive and finite");
+    int dev, sms;
+    int rc = check_arch(&dev, &sms);
+    if (rc) return rc;
+    dim3 grid((T * T + 255) / 256, Nplanes, M);
+    if (elem == 1)
+        bb::extract_tiles_kernel<1><<<grid, 256, 0, (cudaStream_t)stream>>>((const float *)src, Nx, Ny, Nplanes, emitter_positions, M, (double)dx, T, (float *)tiles_out);
+    else
+        bb::extract_tiles_kernel<2><<<grid, 256, 0, (cudaStream_t)stream>>>((const float *)src, Nx, Ny, Nplanes, emitter_positions, M, (double)dx, T, (float *)tiles_out);
+    ++g_launches;
+    BB_CUDA(cudaGetLastError());
+    return BB_OK;
+}
+
+int bb_lightsheet(int Nx, int Ny, float dx, float lambda, float n0, float NA, float z_focus, void *field_out, void *stream) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!field_out) return fail(BB_ERR_INVALID_ARG, "field_out is NULL");
+    if (!(NA > 0.f) || !(dx > 0.f) || !(lambda > 0.f) || !(n0 > 0.f) || !std::isfinite(NA) || !std::isfinite(z_focus))
+        return fail(BB_ERR_INVALID_ARG, "NA, dx, lambda, n0 must be positive and finite, z_focus finite");
+    if (!shape_ok(Nx, Ny))
+        return fail(BB_ERR_UNSUPPORTED_SHAPE, "Nx = %d, Ny = %d: both must be powers of two in [32, 2048], and both >= 256 if one is 2048", Nx, Ny);
+    int dev, sms;
+    int rc = check_arch(&dev, &sms);
+    if (rc) return rc;
+    const double w0 = (double)lambda / (3.14159265358979323846 * (double)NA);
+    bb::gaussian_sheet_kernel<<<dim3((Nx + 127) / 128, Ny), 128, 0, (cudaStream_t)stream>>>((cf *)field_out, Nx, Ny, (double)dx, w0);
+    ++g_launches;
+    BB_CUDA(cudaGetLastError());
+    // back-propagation of the waist by z_focus in the medium n0 (also cuts the evanescent ky, as the definition does)
+    bb_opts o;
+    o.struct_size = (int)sizeof(bb_opts);
+    o.batch = 1;
+    o.nref = nullptr;
+    o.flags = BB_HOMOGENEOUS | (z_focus > 0.f ? BB_BACKWARD : 0u);
+    o.stream = stream;
+    return propagate_impl(field_out, nullptr, Nx, Ny, 1, dx, std::fabs(z_focus), lambda, n0, nullptr, &o, true);
+}
+
+int bb_image_formation(const float *source, int Nx, int Ny, const float *emitter_positions, int M, float dx,
+                       const float *psf_tiles, int T, float *image_out, void *stream) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!source || !emitter_positions || !psf_tiles || !image_out) return fail(BB_ERR_INVALID_ARG, "a pointer argument is NULL");
+    if (Nx < 1 || Ny < 1 || M < 1 || Ny > 65535) return fail(BB_ERR_INVALID_ARG, "Nx, Ny, M must be >= 1 (Ny <= 65535)");
+    if (T < 1 || T > Nx || T > Ny || T > 96) return fail(BB_ERR_INVALID_ARG, "tile size T = %d must be in [1, min(Nx, Ny, 96)]", T);
+    if (!(dx > 0.f) || !std::isfinite(dx)) return fail(BB_ERR_INVALID_ARG, "dx must be positive and finite");
+    int dev, sms;
+    int rc = check_arch(&dev, &sms);
+    if (rc) return rc;
+    DeviceCtx &ctx = device_ctx();
+    rc = ws_reserve(ctx.misc, (size_t)Nx * Ny * sizeof(int));
+    if (rc) return rc;
+    int *owner = (int *)ctx.misc.ptr;
+    cudaStream_t s = (cudaStream_t)stream;
+    bb::nearest_emitter_kernel<<<dim3((Nx + 127) / 128, Ny), 128, 0, s>>>(Nx, Ny, emitter_positions, M, (double)dx, owner);
+    ++g_launches;
+    const size_t smem = (size_t)(32 + T - 1) * (8 + T - 1) * 8;
+    if (smem > 48 * 1024)
+        BB_CUDA(cudaFuncSetAttribute(bb::image_formation_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    bb::image_formation_kernel<<<dim3((Nx + 31) / 32, (Ny + 7) / 8), 256, smem, s>>>(source, owner, Nx, Ny, psf_tiles, T, image_out);
+    ++g_launches;
+    BB_CUDA(cudaGetLastError());
+    return BB_OK;
 }
 
 int bb_propagate_host(void *field_host, const float *dn_host, int Nx, int Ny, int Nz, float dx, float dz,
@@ -675,77 +807,80 @@ int bb_propagate_host(void *field_host, const float *dn_host, int Nx, int Ny, in
     Plan *p;
     rc = get_plan(Nx, Ny, &p);
     if (rc) return rc;
+    DeviceCtx &ctx = device_ctx();
     const float *nref = opts ? opts->nref : nullptr;
     choose_tile_width(p, B, Nz, dx, lambda, n0, nref);
     const size_t npx = (size_t)Nx * Ny;
     const bool per_field = (flags & BB_INTENSITY_PER_FIELD) != 0;
+    const bool backward = (flags & BB_BACKWARD) != 0;
     const int IB = per_field ? B : 1;                        // intensity volumes
     // z-chunks of ~32 MiB of dn, three buffers in flight per direction
     const int NBUF = 3;
     int CZ = (int)std::max<size_t>(1, ((size_t)32 << 20) / (npx * sizeof(float)));
     CZ = std::min(CZ, Nz);
-    rc = ws_reserve(g_ws_field, (size_t)B * npx * sizeof(cf));
-    if (!rc) rc = ws_reserve(g_ws_dn, (size_t)NBUF * CZ * npx * sizeof(float));
-    if (!rc && inten_host) rc = ws_reserve(g_ws_I, (size_t)NBUF * IB * CZ * npx * sizeof(float));
+    rc = ws_reserve(ctx.field, (size_t)B * npx * sizeof(cf));
+    if (!rc && dn_host) rc = ws_reserve(ctx.dn, (size_t)NBUF * CZ * npx * sizeof(float));
+    if (!rc && inten_host) rc = ws_reserve(ctx.I, (size_t)NBUF * IB * CZ * npx * sizeof(float));
     if (rc) return rc;
-    cf *d_field = (cf *)g_ws_field.ptr;
-    float *d_dn = (float *)g_ws_dn.ptr;
-    float *d_I = inten_host ? (float *)g_ws_I.ptr : nullptr;
+    cf *d_field = (cf *)ctx.field.ptr;
+    float *d_dn = dn_host ? (float *)ctx.dn.ptr : nullptr;
+    float *d_I = inten_host ? (float *)ctx.I.ptr : nullptr;
 
-    cudaStream_t s_in, s_run, s_out;
-    BB_CUDA(cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking));
-    BB_CUDA(cudaStreamCreateWithFlags(&s_run, cudaStreamNonBlocking));
-    BB_CUDA(cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking));
+    // streams and events live as long as the library (bb_shutdown releases them)
+    for (cudaStream_t *st : {&ctx.s_in, &ctx.s_run, &ctx.s_out})
+        if (!*st) BB_CUDA(cudaStreamCreateWithFlags(st, cudaStreamNonBlocking));
+    cudaStream_t s_in = ctx.s_in, s_run = ctx.s_run, s_out = ctx.s_out;
     const int nchunks = (Nz + CZ - 1) / CZ;
-    std::vector<cudaEvent_t> ev_in(nchunks), ev_run(nchunks), ev_out(nchunks);
-    for (int c = 0; c < nchunks; ++c) {
-        cudaEventCreateWithFlags(&ev_in[c], cudaEventDisableTiming);
-        cudaEventCreateWithFlags(&ev_run[c], cudaEventDisableTiming);
-        cudaEventCreateWithFlags(&ev_out[c], cudaEventDisableTiming);
+    while ((int)ctx.events.size() < 3 * nchunks) {
+        cudaEvent_t e;
+        BB_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        ctx.events.push_back(e);
     }
+    cudaEvent_t *ev_in = ctx.events.data(), *ev_run = ev_in + nchunks, *ev_out = ev_run + nchunks;
     int result = BB_OK;
-    auto cleanup = [&]() {
-        cudaStreamSynchronize(s_in); cudaStreamSynchronize(s_run); cudaStreamSynchronize(s_out);
-        for (int c = 0; c < nchunks; ++c) { cudaEventDestroy(ev_in[c]); cudaEventDestroy(ev_run[c]); cudaEventDestroy(ev_out[c]); }
-        cudaStreamDestroy(s_in); cudaStreamDestroy(s_run); cudaStreamDestroy(s_out);
-    };
-#define BB_TRY(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { result = fail(BB_ERR_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_)); cleanup(); return result; } } while (0)
+    auto drain = [&]() { cudaStreamSynchronize(s_in); cudaStreamSynchronize(s_run); cudaStreamSynchronize(s_out); };
+#define BB_TRY(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { result = fail(BB_ERR_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_)); drain(); return result; } } while (0)
 
     BB_TRY(cudaMemcpyAsync(d_field, field_host, (size_t)B * npx * sizeof(cf), cudaMemcpyHostToDevice, s_run));
     std::vector<const cf *> h_tab(Nz);
     std::vector<float> h_phase(Nz);
     double k0 = kTwoPi / (double)lambda;
-    float phase_b = (float)(k0 * (double)dz);
-    int prepared = 0;                                        // steps [0, prepared) have tables in place
-    for (int c = 0; c < nchunks; ++c) {
-        const int j0 = c * CZ, j1 = std::min(Nz, j0 + CZ), nz = j1 - j0;
+    float phase_b = (float)(k0 * (double)(backward ? -dz : dz));
+    int prepared = 0;                                        // positions [0, prepared) of the processing order have tables in place
+    for (int c = 0; c < nchunks; ++c) {                      // c counts in processing order: backward runs start at the far end
+        const int zc = backward ? nchunks - 1 - c : c;
+        const int j0 = zc * CZ, j1 = std::min(Nz, j0 + CZ), nz = j1 - j0;
         const int buf = c % NBUF;
-        float *dn_b = d_dn + (size_t)buf * CZ * npx;
+        float *dn_b = d_dn ? d_dn + (size_t)buf * CZ * npx : nullptr;
         float *I_b = d_I ? d_I + (size_t)buf * IB * CZ * npx : nullptr;
-        // dn chunk in: the buffer is free once the chunk that last used it has been computed
-        if (c >= NBUF) BB_TRY(cudaStreamWaitEvent(s_in, ev_run[c - NBUF], 0));
-        BB_TRY(cudaMemcpyAsync(dn_b, dn_host + (size_t)j0 * npx, (size_t)nz * npx * sizeof(float),
-                               cudaMemcpyHostToDevice, s_in));
-        BB_TRY(cudaEventRecord(ev_in[c], s_in));
-        BB_TRY(cudaStreamWaitEvent(s_run, ev_in[c], 0));
+        if (dn_b) {
+            // dn chunk in: the buffer is free once the chunk that last used it has been computed
+            if (c >= NBUF) BB_TRY(cudaStreamWaitEvent(s_in, ev_run[c - NBUF], 0));
+            BB_TRY(cudaMemcpyAsync(dn_b, dn_host + (size_t)j0 * npx, (size_t)nz * npx * sizeof(float),
+                                   cudaMemcpyHostToDevice, s_in));
+            BB_TRY(cudaEventRecord(ev_in[c], s_in));
+            BB_TRY(cudaStreamWaitEvent(s_run, ev_in[c], 0));
+        }
         if (I_b && c >= NBUF) BB_TRY(cudaStreamWaitEvent(s_run, ev_out[c - NBUF], 0));
         if (I_b && (flags & BB_ACCUMULATE)) {                // existing contents are part of the input
             for (int b = 0; b < IB; ++b)
                 BB_TRY(cudaMemcpyAsync(I_b + (size_t)b * CZ * npx, inten_host + ((size_t)b * Nz + j0) * npx,
                                        (size_t)nz * npx * sizeof(float), cudaMemcpyHostToDevice, s_run));
         }
-        int ja = j0;
-        while (ja < j1) {
-            if (ja >= prepared) {
-                rc = prepare_steps(p, B, Nz, ja, dx, dz, lambda, n0, nref, s_run, h_tab, h_phase, &prepared);
-                if (rc || prepared <= ja) { cleanup(); return rc ? rc : fail(BB_ERR_OOM, "propagator table cache too small"); }
+        const int ia = backward ? Nz - j1 : j0, ib = backward ? Nz - j0 : j1;      // positions of this chunk's steps
+        int i = ia;
+        while (i < ib) {
+            if (i >= prepared) {
+                rc = prepare_steps(p, B, Nz, i, dx, dz, lambda, n0, nref, flags, s_run, h_tab, h_phase, &prepared);
+                if (rc || prepared <= i) { drain(); return rc ? rc : fail(BB_ERR_OOM, "propagator table cache too small"); }
             }
-            int jb = std::min(j1, prepared);
-            rc = launch_steps(p, d_field, dn_b + (size_t)(ja - j0) * npx,
+            const int ie = std::min(ib, prepared);
+            const int ja = backward ? Nz - ie : i, jb = backward ? Nz - i : ie;    // the steps of this launch
+            rc = launch_steps(p, d_field, dn_b ? dn_b + (size_t)(ja - j0) * npx : nullptr,
                               I_b ? I_b + (size_t)(ja - j0) * npx : nullptr, (long long)CZ * (long long)npx,
                               B, Nz, ja, jb, phase_b, flags, s_run);
-            if (rc) { cleanup(); return rc; }
-            ja = jb;
+            if (rc) { drain(); return rc; }
+            i = ie;
         }
         BB_TRY(cudaEventRecord(ev_run[c], s_run));
         if (I_b) {
@@ -762,7 +897,6 @@ int bb_propagate_host(void *field_host, const float *dn_host, int Nx, int Ny, in
     BB_TRY(cudaStreamSynchronize(s_in));
     int st = 0;
     BB_TRY(cudaMemcpy(&st, p->status, sizeof st, cudaMemcpyDeviceToHost));
-    cleanup();
 #undef BB_TRY
     if (st != 0) {
         cudaMemset(p->status, 0, sizeof st);
@@ -780,9 +914,10 @@ int bb_nref_from_dn(const float *dn, int Nx, int Ny, int Nz, float n0, int slab,
     if (rc) return rc;
     cudaStream_t s = (cudaStream_t)stream;
     const int NP = 16;
-    rc = ws_reserve(g_ws_misc, (size_t)Nz * NP * sizeof(double));
+    DeviceCtx &ctx = device_ctx();
+    rc = ws_reserve(ctx.misc, (size_t)Nz * NP * sizeof(double));
     if (rc) return rc;
-    double *d_part = (double *)g_ws_misc.ptr;
+    double *d_part = (double *)ctx.misc.ptr;
     size_t npx = (size_t)Nx * Ny;
     for (int j0 = 0; j0 < Nz; j0 += 32768) {                 // gridDim.y limit
         int nz = std::min(32768, Nz - j0);
@@ -812,6 +947,8 @@ int bb_probe_trace(long long *device_buf, int phases) {
     std::lock_guard<std::mutex> lk(g_mu);
     g_trace = device_buf;
     g_trace_phases = device_buf ? phases : 0;
+    g_trace_dev = -1;
+    if (device_buf) cudaGetDevice(&g_trace_dev);
     return BB_OK;
 }
 
@@ -853,11 +990,17 @@ int bb_propagator_table(int Nx, int Ny, float dx, float dz, float lambda, float 
 
 int bb_multiplex_psf(const float *pos, const float *phase, const float *amp, int M, float NA, int Nx, int Ny,
                      float dx, float lambda, void *field_out, void *stream) {
+    return bb_multiplex_annular(pos, phase, amp, M, 0.f, NA, Nx, Ny, dx, lambda, field_out, stream);
+}
+
+int bb_multiplex_annular(const float *pos, const float *phase, const float *amp, int M, float NA_in, float NA, int Nx, int Ny,
+                         float dx, float lambda, void *field_out, void *stream) {
     std::lock_guard<std::mutex> lk(g_mu);
     if (!pos || !field_out) return fail(BB_ERR_INVALID_ARG, "emitter_positions or field_out is NULL");
     if (M < 1) return fail(BB_ERR_INVALID_ARG, "M = %d must be >= 1", M);
     if (!(NA > 0.f) || !(dx > 0.f) || !(lambda > 0.f) || !std::isfinite(NA))
         return fail(BB_ERR_INVALID_ARG, "NA, dx, lambda must be positive and finite");
+    if (!(NA_in >= 0.f) || !(NA_in <= NA)) return fail(BB_ERR_INVALID_ARG, "NA_inner must be in [0, NA]");
     int lx = log2_exact(Nx), ly = log2_exact(Ny);
     if (lx < 5 || lx > 10 || ly < 5 || ly > 10)
         return fail(BB_ERR_UNSUPPORTED_SHAPE, "Nx = %d, Ny = %d: both must be powers of two in [32, 1024]", Nx, Ny);
@@ -867,13 +1010,14 @@ int bb_multiplex_psf(const float *pos, const float *phase, const float *amp, int
     cudaStream_t s = (cudaStream_t)stream;
     // pupil pixel count, in double, same expression as the kernel's inside test
     const double ddx = dx, k0 = kTwoPi / (double)lambda, kc2 = (k0 * (double)NA) * (k0 * (double)NA);
+    const double ki2 = (k0 * (double)NA_in) * (k0 * (double)NA_in);
     long long count = 0;
     std::vector<double> kx2(Nx), ky2(Ny);
     for (int i = 0; i < Nx; ++i) { int f = (i < Nx / 2) ? i : i - Nx; double k = kTwoPi * (double)f / ((double)Nx * ddx); kx2[i] = k * k; }
     for (int i = 0; i < Ny; ++i) { int f = (i < Ny / 2) ? i : i - Ny; double k = kTwoPi * (double)f / ((double)Ny * ddx); ky2[i] = k * k; }
     for (int q = 0; q < Ny; ++q)
         for (int i = 0; i < Nx; ++i)
-            if (kx2[i] + ky2[q] <= kc2) ++count;
+            if (kx2[i] + ky2[q] <= kc2 && kx2[i] + ky2[q] >= ki2) ++count;
     if (count == 0) return fail(BB_ERR_INVALID_ARG, "pupil of NA = %g contains no grid frequency", (double)NA);
     // bounding box of the pupil in DFT bins: [-F, F] per axis, clipped to [-N/2, N/2 - 1]
     auto extent = [&](const std::vector<double> &k2, int N, int *lo, int *w) {
@@ -887,16 +1031,17 @@ int bb_multiplex_psf(const float *pos, const float *phase, const float *amp, int
     extent(kx2, Nx, &Fx, &Wx);
     extent(ky2, Ny, &Fy, &Wy);
     const size_t em_bytes = (((size_t)M * sizeof(bb::EmitterPrep)) + 255) & ~(size_t)255;
-    rc = ws_reserve(g_ws_misc, em_bytes + (size_t)M * (Wx + Wy) * sizeof(cf) + 4096);
+    DeviceCtx &ctx = device_ctx();
+    rc = ws_reserve(ctx.misc, em_bytes + (size_t)M * (Wx + Wy) * sizeof(cf) + 4096);
     if (rc) return rc;
-    bb::EmitterPrep *em = (bb::EmitterPrep *)g_ws_misc.ptr;
-    cf *EX = (cf *)((char *)g_ws_misc.ptr + em_bytes), *EY = EX + (size_t)M * Wx;
+    bb::EmitterPrep *em = (bb::EmitterPrep *)ctx.misc.ptr;
+    cf *EX = (cf *)((char *)ctx.misc.ptr + em_bytes), *EY = EX + (size_t)M * Wx;
     bb::emitter_prep_kernel<<<(M + 127) / 128, 128, 0, s>>>(pos, phase, amp, M, Nx, Ny, ddx, em);
     ++g_launches;
     bb::emitter_axis_kernel<<<dim3((std::max(Wx, Wy) + 127) / 128, M), 128, 0, s>>>(em, M, Fx, Wx, Fy, Wy, EX, EY);
     ++g_launches;
     BB_CUDA(cudaMemsetAsync(field_out, 0, (size_t)Nx * Ny * sizeof(cf), s));
-    bb::multiplex_gemm_kernel<<<dim3((Wx + 31) / 32, (Wy + 31) / 32), 256, 0, s>>>((cf *)field_out, Nx, Ny, ddx, kc2, EX, EY,
+    bb::multiplex_gemm_kernel<<<dim3((Wx + 31) / 32, (Wy + 31) / 32), 256, 0, s>>>((cf *)field_out, Nx, Ny, ddx, ki2, kc2, EX, EY,
                                                                                    M, Fx, Wx, Fy, Wy);
     ++g_launches;
     BB_CUDA(cudaGetLastError());

@@ -85,7 +85,7 @@ __global__ void emitter_axis_kernel(const EmitterPrep *__restrict__ em, int M, i
 
 // U0 over the pupil's bounding box: 32 x 32 outputs per CTA (256 threads, 2 x 2 each), emitters in
 // chunks of 32 through shared memory.  U0 must have been zeroed (pixels outside the box stay zero).
-__global__ void __launch_bounds__(256) multiplex_gemm_kernel(float2 *__restrict__ U0, int Nx, int Ny, double dx, double kc2,
+__global__ void __launch_bounds__(256) multiplex_gemm_kernel(float2 *__restrict__ U0, int Nx, int Ny, double dx, double ki2, double kc2,
                                                              const float2 *__restrict__ EX, const float2 *__restrict__ EY,
                                                              int M, int Fx, int Wx, int Fy, int Wy) {
     const double two_pi = 6.283185307179586476925286766559;
@@ -120,7 +120,8 @@ __global__ void __launch_bounds__(256) multiplex_gemm_kernel(float2 *__restrict_
             const int fq = j - Fy, fp = i - Fx;
             const double kx = __ddiv_rn(__dmul_rn(two_pi, (double)fp), __dmul_rn((double)Nx, dx));
             const double ky = __ddiv_rn(__dmul_rn(two_pi, (double)fq), __dmul_rn((double)Ny, dx));
-            if (!(__dadd_rn(__dmul_rn(kx, kx), __dmul_rn(ky, ky)) <= kc2)) continue;
+            const double k2 = __dadd_rn(__dmul_rn(kx, kx), __dmul_rn(ky, ky));
+            if (!(k2 <= kc2 && k2 >= ki2)) continue;                  // pupil: disk, or annulus (bb_multiplex_annular)
             const int p = fp >= 0 ? fp : fp + Nx, q = fq >= 0 ? fq : fq + Ny;
             U0[(size_t)q * Nx + p] = acc[a][b];
         }
@@ -142,6 +143,82 @@ __global__ void slice_sum_kernel(const float *__restrict__ dn, size_t npx, doubl
         __syncthreads();
     }
     if (threadIdx.x == 0) partial[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = sm[0];
+}
+
+// T x T windows around the emitters of every plane of a stack (bb_extract_tiles): out[e][z][ty][tx] =
+// src[z][(cy - T/2 + ty) mod Ny][(cx - T/2 + tx) mod Nx], (cx, cy) = nearest pixel of emitter e; ELEM floats per pixel.
+template <int ELEM>
+__global__ void extract_tiles_kernel(const float *__restrict__ src, int Nx, int Ny, int Np, const float *__restrict__ pos,
+                                     int M, double dx, int T, float *__restrict__ out) {
+    const int e = blockIdx.z, z = blockIdx.y;
+    const long long cx = (long long)floor(__ddiv_rn((double)pos[2 * e], dx) + 0.5) + Nx / 2;
+    const long long cy = (long long)floor(__ddiv_rn((double)pos[2 * e + 1], dx) + 0.5) + Ny / 2;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < T * T; i += gridDim.x * blockDim.x) {
+        const int ty = i / T, tx = i - ty * T;
+        const long long x = ((cx - T / 2 + tx) % Nx + Nx) % Nx, y = ((cy - T / 2 + ty) % Ny + Ny) % Ny;
+        const float *sp = src + (((size_t)z * Ny + y) * Nx + x) * ELEM;
+        float *op = out + ((((size_t)e * Np + z) * T + ty) * T + tx) * ELEM;
+#pragma unroll
+        for (int c = 0; c < ELEM; ++c) op[c] = sp[c];
+    }
+}
+
+// Waist profile of the cylindrical light sheet (bb_lightsheet): u[y][x] = exp(-y^2 / w0^2), y = (i - Ny/2) dx.
+__global__ void gaussian_sheet_kernel(float2 *__restrict__ u, int Nx, int Ny, double dx, double w0) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x, yi = blockIdx.y;
+    if (x >= Nx) return;
+    const double y = (double)(yi - Ny / 2) * dx;
+    u[(size_t)yi * Nx + x] = make_float2((float)exp(-(y * y) / (w0 * w0)), 0.f);
+}
+
+// Image formation (bb_image_formation), step 1: the emitter nearest to every pixel (periodic distance, lowest
+// index on ties; double, no fused multiply-adds: the comparison is a decision).
+__global__ void nearest_emitter_kernel(int Nx, int Ny, const float *__restrict__ pos, int M, double dx, int *__restrict__ owner) {
+    const int x = blockIdx.x * blockDim.x + threadIdx.x, y = blockIdx.y;
+    if (x >= Nx) return;
+    const double px = __dmul_rn((double)(x - Nx / 2), dx), py = __dmul_rn((double)(y - Ny / 2), dx);
+    const double Lx = __dmul_rn((double)Nx, dx), Ly = __dmul_rn((double)Ny, dx);
+    int best = 0;
+    double bd = 0.0;
+    for (int e = 0; e < M; ++e) {
+        double ddx = __dsub_rn(px, (double)pos[2 * e]), ddy = __dsub_rn(py, (double)pos[2 * e + 1]);
+        ddx = __dsub_rn(ddx, __dmul_rn(Lx, floor(__dadd_rn(__ddiv_rn(ddx, Lx), 0.5))));
+        ddy = __dsub_rn(ddy, __dmul_rn(Ly, floor(__dadd_rn(__ddiv_rn(ddy, Ly), 0.5))));
+        const double d2 = __dadd_rn(__dmul_rn(ddx, ddx), __dmul_rn(ddy, ddy));
+        if (e == 0 || d2 < bd) { bd = d2; best = e; }
+    }
+    owner[(size_t)y * Nx + x] = best;
+}
+
+// Step 2: image[r] = sum over the T x T taps t of S[r - (t - T/2)] psf[owner[r - (t - T/2)]][t] (periodic).
+// A CTA computes a 32 x 8 patch; the (32 + T - 1) x (8 + T - 1) halo of S and owner sits in shared memory.
+__global__ void __launch_bounds__(256) image_formation_kernel(const float *__restrict__ S, const int *__restrict__ owner, int Nx, int Ny,
+                                                              const float *__restrict__ psf, int T, float *__restrict__ image) {
+    extern __shared__ float sm_if[];
+    const int HW = 32 + T - 1, HH = 8 + T - 1;
+    float *sS = sm_if;
+    int *sO = reinterpret_cast<int *>(sm_if + HW * HH);
+    const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 8;
+    // halo origin: source pixel r' = r - (t - T/2) ranges over [r - (T - 1 - T/2), r + T/2]
+    const int hx0 = x0 - (T - 1 - T / 2), hy0 = y0 - (T - 1 - T / 2);
+    for (int i = threadIdx.x; i < HW * HH; i += 256) {
+        const int hy = i / HW, hx = i - hy * HW;
+        const int sx = ((hx0 + hx) % Nx + Nx) % Nx, sy = ((hy0 + hy) % Ny + Ny) % Ny;
+        sS[i] = S[(size_t)sy * Nx + sx];
+        sO[i] = owner[(size_t)sy * Nx + sx];
+    }
+    __syncthreads();
+    const int lx = threadIdx.x % 32, ly = threadIdx.x / 32;
+    const int x = x0 + lx, y = y0 + ly;
+    if (x >= Nx || y >= Ny) return;
+    float acc = 0.f;
+    for (int ty = 0; ty < T; ++ty)
+        for (int tx = 0; tx < T; ++tx) {
+            // r' = r - (t - T/2)  ->  halo index r' - h0 = l + (T - 1 - T/2) - (t - T/2) = l + T - 1 - t
+            const int hi = (ly + T - 1 - ty) * HW + (lx + T - 1 - tx);
+            acc = fmaf(sS[hi], __ldg(psf + ((size_t)sO[hi] * T + ty) * T + tx), acc);
+        }
+    image[(size_t)y * Nx + x] = acc;
 }
 
 }  // namespace bb

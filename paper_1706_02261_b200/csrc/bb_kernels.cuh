@@ -52,6 +52,9 @@ struct KParams {
     unsigned *bar;             // grid barrier counter (zeroed before the launch)
     int *status;               // device flag: != 0 -> watchdog tripped
     unsigned flags;            // BB_ACCUMULATE = 1, BB_INTENSITY_PER_FIELD = 2
+    int backward;              // BB_BACKWARD: steps run from Nz_total - 1 down to 0 (tables and phase offsets are
+                               // conjugated by the host: dz -> -dz)
+    int noscreen;              // BB_HOMOGENEOUS: no phase screen (dn is not read), intensity only
     const int *fmax;           // device [Nz_total]: largest |kx DFT bin| the propagator of step j lets through (conservative)
     int cw4;                   // 16-point-thread kernel: column tiles of 4 columns instead of 8
     int use_tma;               // 16-point-thread kernel: column tiles are fetched by TMA through `tmap`
@@ -62,6 +65,15 @@ struct KParams {
     alignas(64) CUtensorMap tmap;
 };
 
+// Which z-step a phase belongs to.  Forward: row phase r applies the screen of step r - 1 (r >= 1), column
+// phase r the propagator of step r.  Backward (time reversal, Fig. 2c): a step is "x conj screen,
+// FFT2, x conj H, IFFT2", so row phase r applies the screen of step Nz - 1 - r (r < Nz) BEFORE the
+// transform pair that column phase r completes with the table of the same step.
+__device__ __forceinline__ int row_step(const KParams &P, int r) {
+    return P.backward ? (r < P.Nz_total ? P.Nz_total - 1 - r : -1) : r - 1;
+}
+__device__ __forceinline__ int col_step(const KParams &P, int r) { return P.backward ? P.Nz_total - 1 - r : r; }
+
 __device__ __forceinline__ cf ld_cg(const cf *p) { return __ldcg(p); }
 __device__ __forceinline__ void st_cg(cf *p, cf v) { __stcg(p, v); }
 
@@ -70,7 +82,8 @@ struct PhaseDesc {
     bool is_row;
     bool first;        // transform 0 of the phase runs  (row: IFFT_x, column: FFT_y)
     bool second;       // transform 1 of the phase runs  (row: FFT_x,  column: IFFT_y)
-    int kind;          // pointwise factor between the two: 0 none, 1 phase screen of dn slice, 2 table
+    int kind;          // pointwise factor between the two: 0 none, 1 phase screen of dn slice, 2 table,
+                       // 3 no factor but the intensity is recorded (homogeneous medium)
     float scale;
     const void *src;   // kind 1: dn slice (float), kind 2: propagator table (cf)
     float pa;          // kind 1: phase offset k0 dz (n0 - n_ref[j])
@@ -93,17 +106,21 @@ __device__ __forceinline__ PhaseDesc decode_phase(const KParams &P, int p) {
         if (d.is_row) {
             d.first = p >= 2;
             d.second = (p >> 1) < P.Nz_total;
-            if (d.first) {
-                const int j = (p >> 1) - 1;
-                d.kind = 1;
+            const int j = row_step(P, p >> 1);
+            if (j >= 0) {
                 d.slice = (long long)(j - P.j_base) * ((long long)P.Nx * P.Ny);
-                d.src = P.dn + d.slice;
-                d.pa = P.phase_a[j];
+                if (P.noscreen) {
+                    d.kind = 3;
+                } else {
+                    d.kind = 1;
+                    d.src = P.dn + d.slice;
+                    d.pa = P.phase_a[j];
+                }
             }
         } else {
             d.first = true; d.second = true;
             d.kind = 2;
-            d.src = P.htab[p >> 1];
+            d.src = P.htab[col_step(P, p >> 1)];
         }
     } else {
         const PhaseProg &g = P.prog[p];
@@ -237,7 +254,7 @@ __device__ __forceinline__ void run_phase(const KParams &P, const PhaseDesc &d, 
     const Mapping<T, CW> m(P, is_row, sm_y);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const long long npx = (long long)P.Nx * P.Ny;
-    const bool want_I = d.kind == 1 && P.inten != nullptr;
+    const bool want_I = (d.kind == 1 || d.kind == 3) && P.inten != nullptr;
     const bool per_field = (P.flags & 2u) != 0;
     const bool accumulate = (P.flags & 1u) != 0;
     const bool summed = want_I && !per_field && P.B > 1;      // CTA-uniform
@@ -255,7 +272,7 @@ __device__ __forceinline__ void run_phase(const KParams &P, const PhaseDesc &d, 
         }
         // the column transposes synchronise the whole CTA, so there every thread walks through
         if (is_row ? u.valid : cta_has_work) {
-            if (u.valid && d.kind != 0 && (tag.src != d.src || tag.pix0 != u.pix0)) {
+            if (u.valid && (d.kind == 1 || d.kind == 2) && (tag.src != d.src || tag.pix0 != u.pix0)) {
                 fill_pw<T, NX>(d.kind, d.src, u.pix0, d.pa, P.phase_b, pw);
                 tag.src = d.src; tag.pix0 = u.pix0;
             }
@@ -283,13 +300,15 @@ __device__ __forceinline__ void run_phase(const KParams &P, const PhaseDesc &d, 
                 if (pass == 0 && d.kind != 0) {
                     if (is_row) {
                         // u = value * screen, from the conjugate the inverse transform leaves (bb.h step 4)
-                        if (!cj) {
+                        if (d.kind == 3 ? cj : !cj) {
 #pragma unroll
                             for (int i = 0; i < 32; ++i) v[i].y = -v[i].y;
                         }
                         cj = false;
+                        if (d.kind != 3) {
 #pragma unroll
-                        for (int i = 0; i < 32; ++i) v[i] = cmulc(pw[i * kThreads], v[i]);
+                            for (int i = 0; i < 32; ++i) v[i] = cmulc(pw[i * kThreads], v[i]);
+                        }
                         if (want_I) {
                             if (summed) {
 #pragma unroll
@@ -359,7 +378,7 @@ __device__ __forceinline__ void run_phase(const KParams &P, const PhaseDesc &d, 
 // thread's first unit of that phase (they do not depend on the field).
 template <int T, int CW, int NX, int MODE>
 __device__ __forceinline__ void prefill_phase(const KParams &P, const PhaseDesc &d, cf *sm_y, cf *sm_pw, PwTag &tag) {
-    if (d.kind == 0) return;
+    if (d.kind != 1 && d.kind != 2) return;
     const Mapping<T, CW> m(P, MODE == 0 ? d.is_row : MODE == 1, sm_y);
     if (m.n_iter < 1) return;
     const Unit u = m.unit(0);

@@ -38,7 +38,8 @@ struct Smem16 {
 struct Phase16 {
     bool is_row;
     bool first, second;    // first / second transform of the phase runs
-    int kind;              // 0 none, 1 phase screen of a dn slice (+ intensity), 2 propagator table
+    int kind;              // 0 none, 1 phase screen of a dn slice (+ intensity), 2 propagator table,
+                           // 3 intensity only (homogeneous medium)
     const void *src;
     float pa;
     long long slice;       // kind 1: element offset of the intensity slice
@@ -51,17 +52,21 @@ __device__ __forceinline__ Phase16 decode_phase16(const KParams &P, int p) {
     if (d.is_row) {
         d.first = p >= 2;
         d.second = (p >> 1) < P.Nz_total;
-        if (d.first) {
-            const int j = (p >> 1) - 1;
-            d.kind = 1;
+        const int j = row_step(P, p >> 1);
+        if (j >= 0) {
             d.slice = (long long)(j - P.j_base) * ((long long)P.Nx * P.Ny);
-            d.src = P.dn + d.slice;
-            d.pa = P.phase_a[j];
+            if (P.noscreen) {
+                d.kind = 3;
+            } else {
+                d.kind = 1;
+                d.src = P.dn + d.slice;
+                d.pa = P.phase_a[j];
+            }
         }
     } else {
         d.first = d.second = true;
         d.kind = 2;
-        d.src = P.htab[p >> 1];
+        d.src = P.htab[col_step(P, p >> 1)];
     }
     return d;
 }
@@ -392,7 +397,8 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
         // idle column teams stage the screen factors of the next row phase (see stage_screen_by_idle_warps)
         // pstage: the row phase after this column phase (it applies dn slice pstage / 2 - 1), or -1
         const int busy = min(a1 - a0, TM::NTEAM);
-        const void *src_stage = pstage >= 2 ? K.dn + (long long)((pstage >> 1) - 1 - K.j_base) * ((long long)NX * NY) : nullptr;
+        const int jstage = pstage >= 0 && !K.noscreen ? row_step(K, pstage >> 1) : -1;
+        const void *src_stage = jstage >= 0 ? K.dn + (long long)(jstage - K.j_base) * ((long long)NX * NY) : nullptr;
         if (src_stage != nullptr && busy < TM::NTEAM && tagS->src != src_stage) {
             if (tm.team == TM::NTEAM - 1) stage_screen_by_idle_warps<NX / kL, NX, NY, TM::TEAM>(K, decode_phase16(K, pstage), sm_pwS);
             typedef Team16<NX / kL, 1> TR;
@@ -405,7 +411,7 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
     cf *ybuf = sm_y + ((threadIdx.x / (16 * CW)) * (16 * 17 * CW)) + tm.col;        // one region per (team, class)
     cf *xbuf = sm_y + tm.team * (TM::TEAM * 17) + tm.col;                            // same memory, team's part
     cf *pw = sm_pw + threadIdx.x;
-    const bool want_I = d.kind == 1 && K.inten != nullptr;
+    const bool want_I = (d.kind == 1 || d.kind == 3) && K.inten != nullptr;
     const bool accumulate = (K.flags & 1u) != 0;
     // batch kernel: units are (line, field) pairs, fields fastest, so that the teams of a CTA share
     // the pointwise factors of a line; the summed intensity of a row is accumulated in shared
@@ -439,7 +445,7 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
         const int u = ROW ? m : (!BATCH && k == k0 + tm.team ? uc.u0 : LV(Fin, NX, CWL).tile(m));
         if constexpr (BATCH && ROW) {
             pw = sm_pw + (m - a0) * NX;                         // the row's factors, indexed by pixel
-        } else if (d.kind != 0 && (tag.src != d.src || tag.pix0 != u)) {
+        } else if ((d.kind == 1 || d.kind == 2) && (tag.src != d.src || tag.pix0 != u)) {
             fill_pw16<P, CW, ROW, NX>(d.kind, d.src, u, d.pa, K.phase_b, pw);
             tag.src = d.src; tag.pix0 = u;
         }
@@ -504,16 +510,18 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
                 for (int m = 0; m < P; ++m) v[jp * P + m] = ld_cg(line + (tm.q(jp) + kL * m) * NS);
         }
         // v[jp*P + m] is element n = q(jp) + 256 m of the line, in its natural (x- or ky-) order
-        if (d.kind == 1) {
-            // u = value * screen (bb.h step 4), intensity (step 5)
-            if constexpr (BATCH) {
+        if (d.kind == 1 || d.kind == 3) {
+            // u = value * screen (bb.h step 4; not in a homogeneous medium), intensity (step 5)
+            if (d.kind == 1) {
+                if constexpr (BATCH) {
 #pragma unroll
-                for (int jp = 0; jp < JP; ++jp)
+                    for (int jp = 0; jp < JP; ++jp)
 #pragma unroll
-                    for (int mm = 0; mm < P; ++mm) v[jp * P + mm] = cmul(v[jp * P + mm], pw[tm.q(jp) + kL * mm]);
-            } else {
+                        for (int mm = 0; mm < P; ++mm) v[jp * P + mm] = cmul(v[jp * P + mm], pw[tm.q(jp) + kL * mm]);
+                } else {
 #pragma unroll
-                for (int i = 0; i < 16; ++i) v[i] = cmul(v[i], pw[i * kThreads16]);
+                    for (int i = 0; i < 16; ++i) v[i] = cmul(v[i], pw[i * kThreads16]);
+                }
             }
             if (summed) {
                 float *ar = acc + (m - a0) * NX;
@@ -597,7 +605,7 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
 template <int P, int CW, bool ROW, int NX, int NY, bool BATCH>
 __device__ __forceinline__ void prefill_phase16(const KParams &K, const Phase16 &d, cf *sm_pw, PwTag &tag, int Fin) {
     typedef Team16<P, CW> TM;
-    if (d.kind == 0) return;
+    if (d.kind != 1 && d.kind != 2) return;
     if constexpr (BATCH && ROW) {
         if (tag.src != d.src) {
             stage_rows_screen<NX, NY>(K, d, sm_pw);
@@ -651,7 +659,7 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const __grid_const
     // or whose tiles it computes (column phase); fetched one phase ahead so that the global load is not on the critical path
     auto live_in = [&](int p) {
         const bool row = (p & 1) == 0;
-        return row ? ((p >> 1) >= 1 ? P.fmax[(p >> 1) - 1] : NX / 2) : P.fmax[p >> 1];
+        return row ? ((p >> 1) >= 1 ? P.fmax[col_step(P, (p >> 1) - 1)] : NX / 2) : P.fmax[col_step(P, p >> 1)];
     };
     int Fa_next = live_in(P.p0);
     Phase16 d_next = decode_phase16(P, P.p0);
@@ -669,8 +677,9 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const __grid_const
         if (d.is_row && p + 2 < P.p1) {
             // the dn rows this CTA turns into screen factors at the end of this phase (for the row
             // phase after next): start them on their way from HBM to L2 now, one bulk prefetch per row
-            if ((int)threadIdx.x < r1 - r0) {
-                const float *row = P.dn + (long long)((p >> 1) - P.j_base) * ((long long)NX * NY)
+            const int jn = row_step(P, (p >> 1) + 1);
+            if ((int)threadIdx.x < r1 - r0 && jn >= 0 && !P.noscreen) {
+                const float *row = P.dn + (long long)(jn - P.j_base) * ((long long)NX * NY)
                                    + (long long)(r0 + threadIdx.x) * NX;
                 asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(row), "r"(NX * 4) : "memory");
             }
@@ -684,7 +693,7 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const __grid_const
                                                        (!BATCH && p + 1 < P.p1) ? p + 1 : -1, sm_pwS, &tagS);
         }
         if (tracer) tr[1] = clock64();
-        if (BATCH && d.is_row && d.kind == 1 && P.inten != nullptr && !(P.flags & 2u) && P.B > 1)
+        if (BATCH && d.is_row && (d.kind == 1 || d.kind == 3) && P.inten != nullptr && !(P.flags & 2u) && P.B > 1)
             tagH.src = nullptr;                // the intensity sums used the propagator buffer
         if (p + 1 < P.p1) {
             ++nbar;

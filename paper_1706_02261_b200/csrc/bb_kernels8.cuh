@@ -185,7 +185,7 @@ __device__ __forceinline__ void run_phase8(const KParams &K, const Phase16 &d, c
     cf *ybuf = sm_y + (threadIdx.x / (32 * CW)) * (16 * 17 * CW) + tm.col;        // one region per (team, class)
     cf *xbuf = sm_y + tm.team * (TM::TEAM / 32) * (16 * 17) + tm.col;             // same memory, the team's part
     cf *pw = sm_pw + threadIdx.x;
-    const bool want_I = d.kind == 1 && K.inten != nullptr;
+    const bool want_I = (d.kind == 1 || d.kind == 3) && K.inten != nullptr;
     const bool accumulate = (K.flags & 1u) != 0;
     const int B = BATCH ? K.B : 1;
     const long long npx = (long long)NX * NY;
@@ -223,7 +223,7 @@ __device__ __forceinline__ void run_phase8(const KParams &K, const Phase16 &d, c
         const int u = ROW ? m : (!BATCH && k == k0 + tm.team ? uc.u0 : LV(Fin, NX, CWL).tile(m));
         if constexpr (BATCH && ROW) {
             pw = sm_pw + (m - a0) * NX;                         // the row's factors, indexed by pixel
-        } else if (d.kind != 0 && (tag.src != d.src || tag.pix0 != u)) {
+        } else if ((d.kind == 1 || d.kind == 2) && (tag.src != d.src || tag.pix0 != u)) {
             fill_pw8<P, CW, ROW, NX>(d.kind, d.src, u, d.pa, K.phase_b, pw);
             tag.src = d.src; tag.pix0 = u;
         }
@@ -288,14 +288,16 @@ __device__ __forceinline__ void run_phase8(const KParams &K, const Phase16 &d, c
         // P > 1: v[jp*P + m] is element n = q(jp) + 256 m of the line, in its natural (x- or ky-) order;
         // P = 1: v[jj] is element n = t + 16 (4 h + (jj & 3) + 8 (jj >> 2))
         auto pix = [&](int slot) { return tm.pix(slot); };
-        if (d.kind == 1) {
-            // u = value * screen (bb.h step 4), intensity (step 5)
-            if constexpr (BATCH) {
+        if (d.kind == 1 || d.kind == 3) {
+            // u = value * screen (bb.h step 4; not in a homogeneous medium), intensity (step 5)
+            if (d.kind == 1) {
+                if constexpr (BATCH) {
 #pragma unroll
-                for (int i = 0; i < kSlots8; ++i) v[i] = cmul(v[i], pw[pix(i)]);
-            } else {
+                    for (int i = 0; i < kSlots8; ++i) v[i] = cmul(v[i], pw[pix(i)]);
+                } else {
 #pragma unroll
-                for (int i = 0; i < kSlots8; ++i) v[i] = cmul(v[i], pw[i * kThreads8]);
+                    for (int i = 0; i < kSlots8; ++i) v[i] = cmul(v[i], pw[i * kThreads8]);
+                }
             }
             if (summed) {
                 float *ar = acc + (m - a0) * NX;
@@ -368,7 +370,7 @@ __device__ __forceinline__ void run_phase8(const KParams &K, const Phase16 &d, c
 template <int P, int CW, bool ROW, int NX, int NY, bool BATCH>
 __device__ __forceinline__ void prefill_phase8(const KParams &K, const Phase16 &d, cf *sm_pw, PwTag &tag, int Fin) {
     typedef Team8<P, CW> TM;
-    if (d.kind == 0) return;
+    if (d.kind != 1 && d.kind != 2) return;
     if constexpr (BATCH && ROW) {
         if (tag.src != d.src) {
             stage_rows_screen8<NX, NY>(K, d, sm_pw);
@@ -421,7 +423,7 @@ __global__ void __launch_bounds__(kThreads8, 1) bpm8_kernel(const __grid_constan
     UnitCache ucR, ucC;
     auto live_in = [&](int p) {
         const bool row = (p & 1) == 0;
-        return row ? ((p >> 1) >= 1 ? P.fmax[(p >> 1) - 1] : NX / 2) : P.fmax[p >> 1];
+        return row ? ((p >> 1) >= 1 ? P.fmax[col_step(P, (p >> 1) - 1)] : NX / 2) : P.fmax[col_step(P, p >> 1)];
     };
     int Fa_next = live_in(P.p0);
     Phase16 d_next = decode_phase16(P, P.p0);
@@ -437,8 +439,9 @@ __global__ void __launch_bounds__(kThreads8, 1) bpm8_kernel(const __grid_constan
         if (d.is_row && p + 2 < P.p1) {
             // the dn rows this CTA turns into screen factors at the end of this phase (for the row
             // phase after next): start them on their way from HBM to L2 now, one bulk prefetch per row
-            if ((int)threadIdx.x < r1 - r0) {
-                const float *row = P.dn + (long long)((p >> 1) - P.j_base) * ((long long)NX * NY)
+            const int jn = row_step(P, (p >> 1) + 1);
+            if ((int)threadIdx.x < r1 - r0 && jn >= 0 && !P.noscreen) {
+                const float *row = P.dn + (long long)(jn - P.j_base) * ((long long)NX * NY)
                                    + (long long)(r0 + threadIdx.x) * NX;
                 asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(row), "r"(NX * 4) : "memory");
             }
@@ -447,7 +450,7 @@ __global__ void __launch_bounds__(kThreads8, 1) bpm8_kernel(const __grid_constan
         if (d.is_row) run_phase8<PX, 1, true, NX, NY, BATCH>(P, d, sm_tw, sm_twcx, sm_y, sm_pwS, tagS, ucR, Fa, CWC);
         else run_phase8<PY, CWC, false, NX, NY, BATCH>(P, d, sm_tw, sm_twcy, sm_y, sm_pwH, tagH, ucC, Fa, CWC, sm_mbar);
         if (tracer) tr[1] = clock64();
-        if (BATCH && d.is_row && d.kind == 1 && P.inten != nullptr && !(P.flags & 2u) && P.B > 1)
+        if (BATCH && d.is_row && (d.kind == 1 || d.kind == 3) && P.inten != nullptr && !(P.flags & 2u) && P.B > 1)
             tagH.src = nullptr;                // the intensity sums used the propagator buffer
         if (p + 1 < P.p1) {
             ++nbar;
