@@ -23,7 +23,7 @@
  * volumes [Nz][Ny][Nx] float32.  Scalars are float32; every table is built in double from
  * the float32 values promoted to double.  Nx and Ny must be powers of two in [32, 2048]
  * (Nx != Ny allowed; SURVEY 8b asks for [128, 2048], PAPER.md line 31 uses 1024 x 2048); a grid
- * with a 2048-point side needs both sides >= 256, and bb_fft2 / bb_multiplex_* stop at 1024.
+ * with a 2048-point side needs both sides >= 256.
  * Periodic lateral boundaries (plain FFT).
  *
  * Pointers.  Unless a parameter says HOST, pointers are DEVICE pointers on the current CUDA

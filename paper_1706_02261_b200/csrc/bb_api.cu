@@ -406,7 +406,8 @@ int launch_steps(Plan *p, cf *field, const float *dn, float *inten, long long in
                  int Nz_total, int j0, int j1, float phase_b, unsigned flags, cudaStream_t s) {
     KParams P;
     memset(&P, 0, sizeof P);
-    P.field = field; P.dn = dn; P.inten = inten; P.inten_bstride = inten_bstride;
+    P.field = field; P.inten = inten; P.inten_bstride = inten_bstride;
+    P.dn = dn ? dn : reinterpret_cast<const float *>(field);   // BB_HOMOGENEOUS: never read, only tells the slices apart
     P.htab = p->d_htab; P.phase_a = p->d_phase; P.phase_b = phase_b;
     P.Nx = p->Nx; P.Ny = p->Ny; P.B = B; P.BW = batch_warps(B);
     P.Nz_total = Nz_total; P.j_base = j0;
@@ -505,7 +506,17 @@ int run_program(Plan *p, cf *field, int B, const bb::PhaseProg *prog, int nprog,
     P.twx = p->twx; P.twy = p->twy; P.bar = p->bar; P.status = p->status;
     P.p0 = 0; P.p1 = nprog;
     BB_CUDA(cudaMemsetAsync(p->bar, 0, sizeof(unsigned), s));
-    cudaError_t e = bb::kernel_launch(p->Nx, p->Ny, P, p->grid, true, s);
+    cudaError_t e;
+    if (p->k32) {
+        e = bb::kernel_launch(p->Nx, p->Ny, P, p->grid, true, s);
+    } else {
+        // 2048-point lines: the 8-point-thread kernel, rows kept in natural kx order
+        P.tw256 = p->tw256; P.twcx = p->twcx; P.twcy = p->twcy;
+        P.xnat = 1;
+        P.cw4 = p->Ny > 1024 ? 1 : 0;
+        P.use_tma = make_field_tmap(&P.tmap, field, p->Nx, p->Ny, B, P.cw4 ? 4 : 8) ? 1 : 0;
+        e = bb::kernel8_launch(p->Nx, p->Ny, P, p->grid, true, s);
+    }
     ++g_launches;
     if (e != cudaSuccess) return fail(BB_ERR_CUDA, "cooperative launch failed: %s", cudaGetErrorString(e));
     return BB_OK;
@@ -957,9 +968,8 @@ int bb_fft2(void *field, int Nx, int Ny, int batch, int sign, void *stream) {
     if (!field) return fail(BB_ERR_INVALID_ARG, "field is NULL");
     if (batch < 1) return fail(BB_ERR_INVALID_ARG, "batch must be >= 1");
     if (sign != -1 && sign != 1) return fail(BB_ERR_INVALID_ARG, "sign must be -1 or +1");
-    int lx = log2_exact(Nx), ly = log2_exact(Ny);
-    if (lx < 5 || lx > 10 || ly < 5 || ly > 10)
-        return fail(BB_ERR_UNSUPPORTED_SHAPE, "Nx = %d, Ny = %d: both must be powers of two in [32, 1024]", Nx, Ny);
+    if (!shape_ok(Nx, Ny))
+        return fail(BB_ERR_UNSUPPORTED_SHAPE, "Nx = %d, Ny = %d: both must be powers of two in [32, 2048], and both >= 256 if one is 2048", Nx, Ny);
     Plan *p;
     int rc = get_plan(Nx, Ny, &p);
     if (rc) return rc;
@@ -1001,9 +1011,8 @@ int bb_multiplex_annular(const float *pos, const float *phase, const float *amp,
     if (!(NA > 0.f) || !(dx > 0.f) || !(lambda > 0.f) || !std::isfinite(NA))
         return fail(BB_ERR_INVALID_ARG, "NA, dx, lambda must be positive and finite");
     if (!(NA_in >= 0.f) || !(NA_in <= NA)) return fail(BB_ERR_INVALID_ARG, "NA_inner must be in [0, NA]");
-    int lx = log2_exact(Nx), ly = log2_exact(Ny);
-    if (lx < 5 || lx > 10 || ly < 5 || ly > 10)
-        return fail(BB_ERR_UNSUPPORTED_SHAPE, "Nx = %d, Ny = %d: both must be powers of two in [32, 1024]", Nx, Ny);
+    if (!shape_ok(Nx, Ny))
+        return fail(BB_ERR_UNSUPPORTED_SHAPE, "Nx = %d, Ny = %d: both must be powers of two in [32, 2048], and both >= 256 if one is 2048", Nx, Ny);
     Plan *p;
     int rc = get_plan(Nx, Ny, &p);
     if (rc) return rc;

@@ -55,6 +55,7 @@ struct KParams {
     int backward;              // BB_BACKWARD: steps run from Nz_total - 1 down to 0 (tables and phase offsets are
                                // conjugated by the host: dz -> -dz)
     int noscreen;              // BB_HOMOGENEOUS: no phase screen (dn is not read), intensity only
+    int xnat;                  // 8-point-thread kernel, transform programs: rows are in natural kx order in memory
     const int *fmax;           // device [Nz_total]: largest |kx DFT bin| the propagator of step j lets through (conservative)
     int cw4;                   // 16-point-thread kernel: column tiles of 4 columns instead of 8
     int use_tma;               // 16-point-thread kernel: column tiles are fetched by TMA through `tmap`
@@ -69,10 +70,15 @@ struct KParams {
 // phase r the propagator of step r.  Backward (time reversal, Fig. 2c): a step is "x conj screen,
 // FFT2, x conj H, IFFT2", so row phase r applies the screen of step Nz - 1 - r (r < Nz) BEFORE the
 // transform pair that column phase r completes with the table of the same step.
+#ifdef BB_FWD_ONLY
+__device__ __forceinline__ int row_step(const KParams &P, int r) { return r - 1; }
+__device__ __forceinline__ int col_step(const KParams &P, int r) { return r; }
+#else
 __device__ __forceinline__ int row_step(const KParams &P, int r) {
     return P.backward ? (r < P.Nz_total ? P.Nz_total - 1 - r : -1) : r - 1;
 }
 __device__ __forceinline__ int col_step(const KParams &P, int r) { return P.backward ? P.Nz_total - 1 - r : r; }
+#endif
 
 __device__ __forceinline__ cf ld_cg(const cf *p) { return __ldcg(p); }
 __device__ __forceinline__ void st_cg(cf *p, cf v) { __stcg(p, v); }

@@ -38,8 +38,7 @@ struct Smem16 {
 struct Phase16 {
     bool is_row;
     bool first, second;    // first / second transform of the phase runs
-    int kind;              // 0 none, 1 phase screen of a dn slice (+ intensity), 2 propagator table,
-                           // 3 intensity only (homogeneous medium)
+    int kind;              // 0 none, 1 phase screen of a dn slice (+ intensity), 2 propagator table
     const void *src;
     float pa;
     long long slice;       // kind 1: element offset of the intensity slice
@@ -54,14 +53,12 @@ __device__ __forceinline__ Phase16 decode_phase16(const KParams &P, int p) {
         d.second = (p >> 1) < P.Nz_total;
         const int j = row_step(P, p >> 1);
         if (j >= 0) {
+            // (homogeneous medium, KParams::noscreen: dn is a null pointer that is never read -- the staging
+            // functions take dn = 0 -- and d.src only tells the slices apart)
+            d.kind = 1;
             d.slice = (long long)(j - P.j_base) * ((long long)P.Nx * P.Ny);
-            if (P.noscreen) {
-                d.kind = 3;
-            } else {
-                d.kind = 1;
-                d.src = P.dn + d.slice;
-                d.pa = P.phase_a[j];
-            }
+            d.src = P.dn + d.slice;
+            d.pa = P.phase_a[j];
         }
     } else {
         d.first = d.second = true;
@@ -251,7 +248,7 @@ __device__ __forceinline__ cf screen_cossin_small_packed(float r) {
 // kind 2: table value H[n][column] of column tile `unit` (bb.h step 2).  Runs off the critical
 // path where it can (while a grid barrier is pending).
 template <int P, int CW, bool ROW, int NX>
-__device__ __forceinline__ void fill_pw16(int kind, const void *src, int unit, float pa, float pb, cf *pw) {
+__device__ __forceinline__ void fill_pw16(int kind, const void *src, int unit, float pa, float pb, cf *pw, bool noscreen) {
     const Team16<P, CW> tm;
     constexpr int JP = 16 / P;
     if (kind == 1) {
@@ -260,7 +257,7 @@ __device__ __forceinline__ void fill_pw16(int kind, const void *src, int unit, f
 #pragma unroll
         for (int jp = 0; jp < JP; ++jp)
 #pragma unroll
-            for (int m = 0; m < P; ++m) x[jp * P + m] = __ldcs(dnp + tm.q(jp) + kL * m);
+            for (int m = 0; m < P; ++m) x[jp * P + m] = noscreen ? 0.f : __ldcs(dnp + tm.q(jp) + kL * m);
         float amax = 0.f;
 #pragma unroll
         for (int i = 0; i < 16; ++i) {
@@ -303,7 +300,7 @@ __device__ __forceinline__ void stage_rows_screen(const KParams &K, const Phase1
     const float *dnp = reinterpret_cast<const float *>(d.src) + (long long)a0 * NX;
 #pragma unroll 4
     for (int idx = threadIdx.x; idx < total; idx += kThreads16) {
-        const float a = fmaf(K.phase_b, __ldcs(dnp + idx), d.pa);
+        const float a = fmaf(K.phase_b, K.noscreen ? 0.f : __ldcs(dnp + idx), d.pa);
         float s, c;
         if (__all_sync(__activemask(), fabsf(a) <= 0.78539816f)) screen_sincos_small(a, s, c);
         else screen_sincos(a, s, c);
@@ -335,7 +332,7 @@ __device__ __forceinline__ void stage_screen_by_idle_warps(const KParams &K, con
         for (int rl = 0; rl < RCH; ++rl)
 #pragma unroll
             for (int k = 0; k < PER; ++k)
-                x[rl][k] = (rb + rl < rows && s + k * TEAMC < NX) ? __ldcs(dnp + (rb + rl) * NX + k * TEAMC) : 0.f;
+                x[rl][k] = (rb + rl < rows && s + k * TEAMC < NX && !K.noscreen) ? __ldcs(dnp + (rb + rl) * NX + k * TEAMC) : 0.f;
 #pragma unroll
         for (int rl = 0; rl < RCH; ++rl) {
             if (rb + rl < rows) {
@@ -397,7 +394,7 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
         // idle column teams stage the screen factors of the next row phase (see stage_screen_by_idle_warps)
         // pstage: the row phase after this column phase (it applies dn slice pstage / 2 - 1), or -1
         const int busy = min(a1 - a0, TM::NTEAM);
-        const int jstage = pstage >= 0 && !K.noscreen ? row_step(K, pstage >> 1) : -1;
+        const int jstage = pstage >= 0 ? row_step(K, pstage >> 1) : -1;
         const void *src_stage = jstage >= 0 ? K.dn + (long long)(jstage - K.j_base) * ((long long)NX * NY) : nullptr;
         if (src_stage != nullptr && busy < TM::NTEAM && tagS->src != src_stage) {
             if (tm.team == TM::NTEAM - 1) stage_screen_by_idle_warps<NX / kL, NX, NY, TM::TEAM>(K, decode_phase16(K, pstage), sm_pwS);
@@ -411,7 +408,7 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
     cf *ybuf = sm_y + ((threadIdx.x / (16 * CW)) * (16 * 17 * CW)) + tm.col;        // one region per (team, class)
     cf *xbuf = sm_y + tm.team * (TM::TEAM * 17) + tm.col;                            // same memory, team's part
     cf *pw = sm_pw + threadIdx.x;
-    const bool want_I = (d.kind == 1 || d.kind == 3) && K.inten != nullptr;
+    const bool want_I = d.kind == 1 && K.inten != nullptr;
     const bool accumulate = (K.flags & 1u) != 0;
     // batch kernel: units are (line, field) pairs, fields fastest, so that the teams of a CTA share
     // the pointwise factors of a line; the summed intensity of a row is accumulated in shared
@@ -445,8 +442,8 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
         const int u = ROW ? m : (!BATCH && k == k0 + tm.team ? uc.u0 : LV(Fin, NX, CWL).tile(m));
         if constexpr (BATCH && ROW) {
             pw = sm_pw + (m - a0) * NX;                         // the row's factors, indexed by pixel
-        } else if ((d.kind == 1 || d.kind == 2) && (tag.src != d.src || tag.pix0 != u)) {
-            fill_pw16<P, CW, ROW, NX>(d.kind, d.src, u, d.pa, K.phase_b, pw);
+        } else if (d.kind != 0 && (tag.src != d.src || tag.pix0 != u)) {
+            fill_pw16<P, CW, ROW, NX>(d.kind, d.src, u, d.pa, K.phase_b, pw, K.noscreen != 0);
             tag.src = d.src; tag.pix0 = u;
         }
         cf *line = K.field + b * npx + (ROW ? (long long)u * NX : (long long)u * CW + tm.col);
@@ -510,18 +507,16 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
                 for (int m = 0; m < P; ++m) v[jp * P + m] = ld_cg(line + (tm.q(jp) + kL * m) * NS);
         }
         // v[jp*P + m] is element n = q(jp) + 256 m of the line, in its natural (x- or ky-) order
-        if (d.kind == 1 || d.kind == 3) {
-            // u = value * screen (bb.h step 4; not in a homogeneous medium), intensity (step 5)
-            if (d.kind == 1) {
-                if constexpr (BATCH) {
+        if (d.kind == 1) {
+            // u = value * screen (bb.h step 4), intensity (step 5)
+            if constexpr (BATCH) {
 #pragma unroll
-                    for (int jp = 0; jp < JP; ++jp)
+                for (int jp = 0; jp < JP; ++jp)
 #pragma unroll
-                        for (int mm = 0; mm < P; ++mm) v[jp * P + mm] = cmul(v[jp * P + mm], pw[tm.q(jp) + kL * mm]);
-                } else {
+                    for (int mm = 0; mm < P; ++mm) v[jp * P + mm] = cmul(v[jp * P + mm], pw[tm.q(jp) + kL * mm]);
+            } else {
 #pragma unroll
-                    for (int i = 0; i < 16; ++i) v[i] = cmul(v[i], pw[i * kThreads16]);
-                }
+                for (int i = 0; i < 16; ++i) v[i] = cmul(v[i], pw[i * kThreads16]);
             }
             if (summed) {
                 float *ar = acc + (m - a0) * NX;
@@ -605,7 +600,7 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
 template <int P, int CW, bool ROW, int NX, int NY, bool BATCH>
 __device__ __forceinline__ void prefill_phase16(const KParams &K, const Phase16 &d, cf *sm_pw, PwTag &tag, int Fin) {
     typedef Team16<P, CW> TM;
-    if (d.kind != 1 && d.kind != 2) return;
+    if (d.kind == 0) return;
     if constexpr (BATCH && ROW) {
         if (tag.src != d.src) {
             stage_rows_screen<NX, NY>(K, d, sm_pw);
@@ -626,7 +621,7 @@ __device__ __forceinline__ void prefill_phase16(const KParams &K, const Phase16 
     const int m = BATCH ? k / B : k;
     const int u = ROW ? m : lv.tile(m);
     if (tag.src == d.src && tag.pix0 == u) return;
-    fill_pw16<P, CW, ROW, NX>(d.kind, d.src, u, d.pa, K.phase_b, sm_pw + threadIdx.x);
+    fill_pw16<P, CW, ROW, NX>(d.kind, d.src, u, d.pa, K.phase_b, sm_pw + threadIdx.x, K.noscreen != 0);
     tag.src = d.src; tag.pix0 = u;
 }
 
@@ -690,10 +685,14 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const __grid_const
             run_phase16<PX, 1, true, NX, NY, BATCH>(P, d, sm_tw, sm_twcx, sm_y, sm_pwS, tagS, ucR, Fa, CWC);
         } else {
             run_phase16<PY, CWC, false, NX, NY, BATCH>(P, d, sm_tw, sm_twcy, sm_y, sm_pwH, tagH, ucC, Fa, CWC, sm_mbar,
+#ifdef BB_NO_IDLE_STAGING
+                                                       -1, sm_pwS, &tagS);
+#else
                                                        (!BATCH && p + 1 < P.p1) ? p + 1 : -1, sm_pwS, &tagS);
+#endif
         }
         if (tracer) tr[1] = clock64();
-        if (BATCH && d.is_row && (d.kind == 1 || d.kind == 3) && P.inten != nullptr && !(P.flags & 2u) && P.B > 1)
+        if (BATCH && d.is_row && d.kind == 1 && P.inten != nullptr && !(P.flags & 2u) && P.B > 1)
             tagH.src = nullptr;                // the intensity sums used the propagator buffer
         if (p + 1 < P.p1) {
             ++nbar;
@@ -711,7 +710,11 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const __grid_const
                 prefill_phase16<PY, CWC, false, NX, NY, BATCH>(P, d_next, sm_pwH, tagH, Fn);
                 // screen factors of the row phase after next: here, unless the coming column phase has
                 // idle warps for them (same live band as the last column phase, which had an idle team)
+#ifdef BB_NO_IDLE_STAGING
+                const bool col_stages = false;
+#else
                 const bool col_stages = !BATCH && ucC.F == Fn && (ucC.a1 - ucC.a0) < Team16<PY, CWC>::NTEAM;
+#endif
                 if (p + 2 < P.p1 && !col_stages) prefill_phase16<PX, 1, true, NX, NY, BATCH>(P, decode_phase16(P, p + 2), sm_pwS, tagS, 0);
             } else {
                 prefill_phase16<PX, 1, true, NX, NY, BATCH>(P, d_next, sm_pwS, tagS, 0);

@@ -97,13 +97,13 @@ __device__ __forceinline__ void class_dft_any(cf *w) {
 // kind 1: exp(i (pb dn + pa)) at pixel n = q(jp) + 256 m of row `unit` of a dn slice (bb.h step 4);
 // kind 2: table value H[n][column] of column tile `unit` (bb.h step 2).
 template <int P, int CW, bool ROW, int NX>
-__device__ __forceinline__ void fill_pw8(int kind, const void *src, int unit, float pa, float pb, cf *pw) {
+__device__ __forceinline__ void fill_pw8(int kind, const void *src, int unit, float pa, float pb, cf *pw, bool noscreen) {
     const Team8<P, CW> tm;
     if (kind == 1) {
         const float *dnp = reinterpret_cast<const float *>(src) + (long long)unit * NX;
         float x[kSlots8];
 #pragma unroll
-        for (int i = 0; i < kSlots8; ++i) x[i] = __ldcs(dnp + tm.pix(i));
+        for (int i = 0; i < kSlots8; ++i) x[i] = noscreen ? 0.f : __ldcs(dnp + tm.pix(i));
         float amax = 0.f;
 #pragma unroll
         for (int i = 0; i < kSlots8; ++i) {
@@ -142,7 +142,7 @@ __device__ __forceinline__ void stage_rows_screen8(const KParams &K, const Phase
     const float *dnp = reinterpret_cast<const float *>(d.src) + (long long)a0 * NX;
 #pragma unroll 4
     for (int idx = threadIdx.x; idx < total; idx += kThreads8) {
-        const float a = fmaf(K.phase_b, __ldcs(dnp + idx), d.pa);
+        const float a = fmaf(K.phase_b, K.noscreen ? 0.f : __ldcs(dnp + idx), d.pa);
         float s, c;
         if (__all_sync(__activemask(), fabsf(a) <= 0.78539816f)) screen_sincos_small(a, s, c);
         else screen_sincos(a, s, c);
@@ -157,13 +157,15 @@ __device__ __forceinline__ void stage_rows_screen8(const KParams &K, const Phase
 template <int P, int CW, bool ROW, int NX, int NY, bool BATCH>
 __device__ __forceinline__ void run_phase8(const KParams &K, const Phase16 &d, const cf *sm_tw, const cf *sm_twc,
                                            cf *sm_y, cf *sm_pw, PwTag &tag, UnitCache &uc, int Fin, int cwc,
-                                           unsigned long long *sm_mbar = nullptr) {
+                                           unsigned long long *sm_mbar = nullptr, float scale = 1.f) {
     typedef Team8<P, CW> TM;
     constexpr int S1 = ROW ? +1 : -1, S2 = -S1;
     constexpr int JP = TM::JP;
     constexpr long long NS = ROW ? 1 : NX;               // element stride of the line index
     constexpr long long CS = ROW ? kL : NX;              // class stride: class-major (rows) / interleaved (columns)
     constexpr long long IS = ROW ? 1 : (long long)P * NX;   // stride inside a class
+    // transform programs (bb_fft2, bb_multiplex_*) keep kx in natural order: class c, index k' at P k' + c
+    const long long CSr = (ROW && K.xnat) ? 1 : CS, ISr = (ROW && K.xnat) ? P : IS;
     const TM tm;
     if (tm.team >= TM::NTEAM) return;
     constexpr int CWL = CW == 8 ? 3 : (CW == 4 ? 2 : 0);
@@ -185,7 +187,7 @@ __device__ __forceinline__ void run_phase8(const KParams &K, const Phase16 &d, c
     cf *ybuf = sm_y + (threadIdx.x / (32 * CW)) * (16 * 17 * CW) + tm.col;        // one region per (team, class)
     cf *xbuf = sm_y + tm.team * (TM::TEAM / 32) * (16 * 17) + tm.col;             // same memory, the team's part
     cf *pw = sm_pw + threadIdx.x;
-    const bool want_I = (d.kind == 1 || d.kind == 3) && K.inten != nullptr;
+    const bool want_I = d.kind == 1 && K.inten != nullptr;
     const bool accumulate = (K.flags & 1u) != 0;
     const int B = BATCH ? K.B : 1;
     const long long npx = (long long)NX * NY;
@@ -197,7 +199,7 @@ __device__ __forceinline__ void run_phase8(const KParams &K, const Phase16 &d, c
         if (d.kind == 1 && tag.src != d.src) {                 // not staged during the barrier
             asm volatile("bar.sync 15, %0;" ::"n"(NW) : "memory");
             for (int idx = threadIdx.x; idx < (a1 - a0) * NX; idx += NW) {
-                const float a = fmaf(K.phase_b, __ldcs(reinterpret_cast<const float *>(d.src) + (long long)a0 * NX + idx), d.pa);
+                const float a = fmaf(K.phase_b, K.noscreen ? 0.f : __ldcs(reinterpret_cast<const float *>(d.src) + (long long)a0 * NX + idx), d.pa);
                 float s, c;
                 screen_sincos(a, s, c);
                 sm_pw[idx] = make_float2(c, s);
@@ -223,8 +225,8 @@ __device__ __forceinline__ void run_phase8(const KParams &K, const Phase16 &d, c
         const int u = ROW ? m : (!BATCH && k == k0 + tm.team ? uc.u0 : LV(Fin, NX, CWL).tile(m));
         if constexpr (BATCH && ROW) {
             pw = sm_pw + (m - a0) * NX;                         // the row's factors, indexed by pixel
-        } else if ((d.kind == 1 || d.kind == 2) && (tag.src != d.src || tag.pix0 != u)) {
-            fill_pw8<P, CW, ROW, NX>(d.kind, d.src, u, d.pa, K.phase_b, pw);
+        } else if (d.kind != 0 && (tag.src != d.src || tag.pix0 != u)) {
+            fill_pw8<P, CW, ROW, NX>(d.kind, d.src, u, d.pa, K.phase_b, pw, K.noscreen != 0);
             tag.src = d.src; tag.pix0 = u;
         }
         cf *line = K.field + b * npx + (ROW ? (long long)u * NX : (long long)u * CW + tm.col);
@@ -252,11 +254,11 @@ __device__ __forceinline__ void run_phase8(const KParams &K, const Phase16 &d, c
         }
         if (d.first) {
             if (!loaded) {
-                const cf *src = line + tm.c * CS + (16 * tm.l.h + tm.l.t) * IS;
+                const cf *src = line + tm.c * CSr + (16 * tm.l.h + tm.l.t) * ISr;
 #pragma unroll
                 for (int i = 0; i < kSlots8; ++i) {
                     v[i] = make_float2(0.f, 0.f);
-                    if (!ROW || ((lmask >> (2 * i)) & 1u)) v[i] = ld_cg(src + 32 * IS * i);
+                    if (!ROW || ((lmask >> (2 * i)) & 1u)) v[i] = ld_cg(src + 32 * ISr * i);
                 }
             }
             if constexpr (ROW) subline8_dit<S1, CW>(v, sm_tw, ybuf, tm.l, wsync);
@@ -288,16 +290,14 @@ __device__ __forceinline__ void run_phase8(const KParams &K, const Phase16 &d, c
         // P > 1: v[jp*P + m] is element n = q(jp) + 256 m of the line, in its natural (x- or ky-) order;
         // P = 1: v[jj] is element n = t + 16 (4 h + (jj & 3) + 8 (jj >> 2))
         auto pix = [&](int slot) { return tm.pix(slot); };
-        if (d.kind == 1 || d.kind == 3) {
-            // u = value * screen (bb.h step 4; not in a homogeneous medium), intensity (step 5)
-            if (d.kind == 1) {
-                if constexpr (BATCH) {
+        if (d.kind == 1) {
+            // u = value * screen (bb.h step 4), intensity (step 5)
+            if constexpr (BATCH) {
 #pragma unroll
-                    for (int i = 0; i < kSlots8; ++i) v[i] = cmul(v[i], pw[pix(i)]);
-                } else {
+                for (int i = 0; i < kSlots8; ++i) v[i] = cmul(v[i], pw[pix(i)]);
+            } else {
 #pragma unroll
-                    for (int i = 0; i < kSlots8; ++i) v[i] = cmul(v[i], pw[i * kThreads8]);
-                }
+                for (int i = 0; i < kSlots8; ++i) v[i] = cmul(v[i], pw[i * kThreads8]);
             }
             if (summed) {
                 float *ar = acc + (m - a0) * NX;
@@ -318,6 +318,10 @@ __device__ __forceinline__ void run_phase8(const KParams &K, const Phase16 &d, c
             // U * H (bb.h step 2)
 #pragma unroll
             for (int i = 0; i < kSlots8; ++i) v[i] = cmul(v[i], pw[i * kThreads8]);
+        }
+        if (scale != 1.f) {
+#pragma unroll
+            for (int i = 0; i < kSlots8; ++i) v[i] = make_float2(v[i].x * scale, v[i].y * scale);
         }
         if (d.second) {
             if constexpr (P > 1) {
@@ -341,9 +345,9 @@ __device__ __forceinline__ void run_phase8(const KParams &K, const Phase16 &d, c
             tm.sync();                                      // region free again for the transposes
             if constexpr (ROW) subline8_dif<S2, CW>(v, sm_tw, ybuf, tm.l, wsync);
             else subline8_dif<S2, CW>(v, sm_tw, ybuf, tm.l, gsync);
-            cf *dst = line + tm.c * CS + (16 * tm.l.h + tm.l.t) * IS;
+            cf *dst = line + tm.c * CSr + (16 * tm.l.h + tm.l.t) * ISr;
 #pragma unroll
-            for (int i = 0; i < kSlots8; ++i) st_cg(dst + 32 * IS * i, v[i]);
+            for (int i = 0; i < kSlots8; ++i) st_cg(dst + 32 * ISr * i, v[i]);
         } else {
 #pragma unroll
             for (int i = 0; i < kSlots8; ++i) st_cg(line + (long long)pix(i) * NS, v[i]);
@@ -370,7 +374,7 @@ __device__ __forceinline__ void run_phase8(const KParams &K, const Phase16 &d, c
 template <int P, int CW, bool ROW, int NX, int NY, bool BATCH>
 __device__ __forceinline__ void prefill_phase8(const KParams &K, const Phase16 &d, cf *sm_pw, PwTag &tag, int Fin) {
     typedef Team8<P, CW> TM;
-    if (d.kind != 1 && d.kind != 2) return;
+    if (d.kind == 0) return;
     if constexpr (BATCH && ROW) {
         if (tag.src != d.src) {
             stage_rows_screen8<NX, NY>(K, d, sm_pw);
@@ -392,7 +396,7 @@ __device__ __forceinline__ void prefill_phase8(const KParams &K, const Phase16 &
     const int m = BATCH ? k / B : k;
     const int u = ROW ? m : lv.tile(m);
     if (tag.src == d.src && tag.pix0 == u) return;
-    fill_pw8<P, CW, ROW, NX>(d.kind, d.src, u, d.pa, K.phase_b, sm_pw + threadIdx.x);
+    fill_pw8<P, CW, ROW, NX>(d.kind, d.src, u, d.pa, K.phase_b, sm_pw + threadIdx.x, K.noscreen != 0);
     tag.src = d.src; tag.pix0 = u;
 }
 
@@ -422,11 +426,22 @@ __global__ void __launch_bounds__(kThreads8, 1) bpm8_kernel(const __grid_constan
     PwTag tagH = {nullptr, -1}, tagS = {nullptr, -1};
     UnitCache ucR, ucC;
     auto live_in = [&](int p) {
+        if (P.mode == 1) return NX / 2;                       // transform programs: every column is live
         const bool row = (p & 1) == 0;
         return row ? ((p >> 1) >= 1 ? P.fmax[col_step(P, (p >> 1) - 1)] : NX / 2) : P.fmax[col_step(P, p >> 1)];
     };
+    // mode 1 (bb_fft2, bb_multiplex_*): phase p is the line transform KParams::prog[p] describes
+    auto decode = [&](int p) {
+        if (P.mode == 0) return decode_phase16(P, p);
+        Phase16 d;
+        d.kind = 0; d.src = nullptr; d.pa = 0.f; d.slice = 0;
+        d.is_row = P.prog[p].is_row != 0;
+        d.first = d.is_row ? P.prog[p].inv != 0 : P.prog[p].fwd != 0;
+        d.second = d.is_row ? P.prog[p].fwd != 0 : P.prog[p].inv != 0;
+        return d;
+    };
     int Fa_next = live_in(P.p0);
-    Phase16 d_next = decode_phase16(P, P.p0);
+    Phase16 d_next = decode(P.p0);
     const int r0 = (int)((unsigned)NY * blockIdx.x / gridDim.x);          // rows of this CTA (row phases)
     const int r1 = (int)((unsigned)NY * (blockIdx.x + 1) / gridDim.x);
     unsigned nbar = 0;
@@ -436,7 +451,7 @@ __global__ void __launch_bounds__(kThreads8, 1) bpm8_kernel(const __grid_constan
     for (int p = P.p0; p < P.p1; ++p) {
         const Phase16 d = d_next;              // decoded while the previous barrier was pending
         if (tracer) tr[0] = clock64();
-        if (d.is_row && p + 2 < P.p1) {
+        if (d.is_row && p + 2 < P.p1 && P.mode == 0) {
             // the dn rows this CTA turns into screen factors at the end of this phase (for the row
             // phase after next): start them on their way from HBM to L2 now, one bulk prefetch per row
             const int jn = row_step(P, (p >> 1) + 1);
@@ -447,18 +462,20 @@ __global__ void __launch_bounds__(kThreads8, 1) bpm8_kernel(const __grid_constan
             }
         }
         const int Fa = Fa_next;
-        if (d.is_row) run_phase8<PX, 1, true, NX, NY, BATCH>(P, d, sm_tw, sm_twcx, sm_y, sm_pwS, tagS, ucR, Fa, CWC);
-        else run_phase8<PY, CWC, false, NX, NY, BATCH>(P, d, sm_tw, sm_twcy, sm_y, sm_pwH, tagH, ucC, Fa, CWC, sm_mbar);
+        const float scale = P.mode == 1 ? P.prog[p].scale : 1.f;
+        if (d.is_row) run_phase8<PX, 1, true, NX, NY, BATCH>(P, d, sm_tw, sm_twcx, sm_y, sm_pwS, tagS, ucR, Fa, CWC, nullptr, scale);
+        else run_phase8<PY, CWC, false, NX, NY, BATCH>(P, d, sm_tw, sm_twcy, sm_y, sm_pwH, tagH, ucC, Fa, CWC, sm_mbar, scale);
         if (tracer) tr[1] = clock64();
-        if (BATCH && d.is_row && (d.kind == 1 || d.kind == 3) && P.inten != nullptr && !(P.flags & 2u) && P.B > 1)
+        if (BATCH && d.is_row && d.kind == 1 && P.inten != nullptr && !(P.flags & 2u) && P.B > 1)
             tagH.src = nullptr;                // the intensity sums used the propagator buffer
         if (p + 1 < P.p1) {
             ++nbar;
             grid_arrive(P.bar);
             if (tracer) tr[2] = clock64();
             Fa_next = live_in(p + 1);
-            d_next = decode_phase16(P, p + 1);   // its global loads (table pointer, phase offset) overlap the barrier
-            if (d.is_row) {
+            d_next = decode(p + 1);   // its global loads (table pointer, phase offset) overlap the barrier
+            if (P.mode == 1) {
+            } else if (d.is_row) {
                 const int Fn = Fa_next;
                 prefill_phase8<PY, CWC, false, NX, NY, BATCH>(P, d_next, sm_pwH, tagH, Fn);
                 if (p + 2 < P.p1) prefill_phase8<PX, 1, true, NX, NY, BATCH>(P, decode_phase16(P, p + 2), sm_pwS, tagS, 0);

@@ -16,7 +16,8 @@ FFT_TOL = 5e-7
 
 @pytest.mark.parametrize("Nx,Ny,B", [(32, 32, 1), (64, 32, 3), (32, 128, 2), (128, 128, 1), (256, 64, 2),
                                       (512, 256, 1), (256, 512, 2), (1024, 128, 1), (128, 1024, 1),
-                                      (512, 512, 5), (1024, 1024, 2)])
+                                      (512, 512, 5), (1024, 1024, 2),
+                                      (2048, 1024, 1), (1024, 2048, 1), (2048, 2048, 1), (2048, 256, 2), (256, 2048, 1)])
 def test_fft2_matches_oracle(oracle_mod, Nx, Ny, B):
     bb = need_gpu()
     f = wl.random_field(Nx, Ny, seed=Nx * 7 + Ny, batch=B)
@@ -101,6 +102,10 @@ def test_multiplex_psf_defaults_subpixel_and_nonsquare(oracle_mod):
     pos = rng.uniform(-5, 5, size=(7, 2)).astype(np.float32)      # off-grid positions
     ref = oracle_mod.multiplex_psf(pos, None, None, 0.6, 256, 128, 0.15, 0.5)
     got = bb.multiplex_psf(torch.from_numpy(pos).cuda(), None, None, 0.6, 256, 128, 0.15, 0.5)
+    assert rel_l2(got.cpu().numpy(), ref) < 2e-6
+    # the paper's own lateral grid (1024 x 2048): 2048-point lines
+    ref = oracle_mod.multiplex_psf(pos, None, None, 0.8, 2048, 1024, 0.1, 0.5)
+    got = bb.multiplex_psf(torch.from_numpy(pos).cuda(), None, None, 0.8, 2048, 1024, 0.1, 0.5)
     assert rel_l2(got.cpu().numpy(), ref) < 2e-6
     one = np.zeros((1, 2), dtype=np.float32)                      # on-grid unit emitter: value 1 at its pixel
     got = bb.multiplex_psf(torch.from_numpy(one).cuda(), None, None, 0.8, 128, 128, 0.1, 0.5).cpu().numpy()

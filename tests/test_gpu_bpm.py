@@ -50,7 +50,8 @@ def run_both(bb, oracle, w, dn, f0, nref, flags=0, intensity_init=None):
 
 @pytest.mark.parametrize("Nx,Ny,Nz,B", [(32, 32, 5, 1), (64, 128, 7, 1), (128, 64, 6, 2), (256, 32, 4, 3),
                                          (32, 512, 3, 1), (512, 128, 5, 1), (1024, 64, 3, 2), (64, 1024, 3, 1),
-                                         (256, 256, 9, 5), (512, 512, 4, 9), (1024, 1024, 3, 1)])
+                                         (256, 256, 9, 5), (512, 512, 4, 9), (1024, 1024, 3, 1),
+                                         (2048, 1024, 2, 1), (1024, 2048, 2, 1), (2048, 2048, 2, 1)])
 def test_small_shapes_batches_and_ragged_tiles(oracle_mod, Nx, Ny, Nz, B):
     """Every line length, non-square grids, batches that do not divide the warps, grids whose
     tiles do not divide the CTAs (ragged tail), with an adapted n_ref that changes every 2 slices."""
