@@ -52,13 +52,17 @@ def measured_peaks():
 
 def committed_dram_traffic(workload: str):
     """DRAM bytes per launch of the persistent kernel from the committed ncu capture
-    (profiles/dram_traffic.csv; the command that made it is in the file it names), or None."""
+    (profiles/dram_traffic.csv; the command that made it is in the file it names) -- but only if that
+    capture was taken from the library source that is being timed now (its digest is in the row);
+    otherwise None: a traffic figure of another build would be a claim about code that is not running."""
     import csv
+    from paper_1706_02261_b200 import build
     p = os.path.join(ROOT, "profiles", "dram_traffic.csv")
     try:
+        digest = build._digest(build._sources())
         with open(p) as f:
             for row in csv.DictReader(f):
-                if row["workload"] == workload:
+                if row["workload"] == workload and row.get("source_digest", "") == digest:
                     return int(row["dram_bytes_per_launch"])
     except Exception:
         pass
@@ -73,6 +77,20 @@ def algorithmic_per_step(w: wl.Workload, per_field_intensity=False):
     l2 = 32 * npx * B + 8 * npx + hbm
     flops = (10 * npx * (math.log2(w.Nx) + math.log2(w.Ny)) + 40 * npx) * B
     return hbm, l2, flops
+
+
+def roofline_fracs(w, dur_s, peaks, per_field=False):
+    """T_roof / T and the three fractions for a propagation of w.Nz steps that took dur_s."""
+    hbm_b, l2_b, flop = algorithmic_per_step(w, per_field)
+    t = dur_s / w.Nz
+    out = {"us_per_z_step": t * 1e6,
+           "hbm_frac": hbm_b / (peaks["hbm"] * 1e9) / t,
+           "alu_frac": flop / (FP32_PEAK_TFLOPS * 1e12) / t}
+    if peaks.get("l2_copy"):
+        out["l2_frac"] = l2_b / (peaks["l2_copy"] * 1e9) / t
+        out["l2_frac_vs_read_peak"] = l2_b / (peaks["l2_read"] * 1e9) / t
+        out["hbm_l2_roofline_frac"] = max(hbm_b / (peaks["hbm"] * 1e9), l2_b / (peaks["l2_copy"] * 1e9)) / t
+    return out
 
 
 class ClockSampler:
@@ -133,10 +151,70 @@ def make_inputs(w: wl.Workload, device):
 
 
 # --------------------------------------------------------------------------------------------
+def flush_l2(scratch):
+    """A 256 MiB write between timed runs, so that a small dn volume is not found in the 126 MB L2."""
+    scratch.add_(1.0)
+
+
+def time_propagation(bb, w, dev, field0_fn, dn, nref, inten, flags=0, runs=10, warmup=3, scratch=None):
+    """CUDA-event times (ms) of `runs` propagations of workload w, each from a fresh input field."""
+    field = field0_fn()
+    ts = []
+    for i in range(warmup + runs):
+        field = field0_fn(field)
+        if scratch is not None:
+            flush_l2(scratch)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        bb.propagate(field, dn, w.dx, w.dz, w.lam, w.n0, intensity=inten, nref=nref, flags=flags)
+        b.record()
+        torch.cuda.synchronize()
+        if i >= warmup:
+            ts.append(a.elapsed_time(b))
+    return ts
+
+
+def time_config(bb, dev, name, peaks, scratch, per_field=False, runs=10):
+    """One entry of the `configs` array: a parity-test configuration timed the way SURVEY 8d asks
+    (3 warm-ups, median and min of >= 10 runs, L2 flushed in between, plan and tables resident)."""
+    w = wl.config(name)
+    dn, f0, em = make_inputs(w, dev)
+    nref = bb.nref_from_dn(dn, w.n0, w.nref_slab).numpy()
+    if em is not None:
+        em_d = tuple(t.to(dev) for t in em)
+        src = bb.multiplex_psf(em_d[0], em_d[1], em_d[2], w.NA, w.Nx, w.Ny, w.dx, w.lam)[None].contiguous()
+    else:
+        src = torch.from_numpy(f0).to(dev)
+
+    def field0(buf=None):
+        if buf is None:
+            return src.clone()
+        buf.copy_(src)
+        return buf
+
+    B = w.batch
+    flags = bb.INTENSITY_PER_FIELD if per_field else 0
+    inten = torch.empty(((B,) if per_field else ()) + (w.Nz, w.Ny, w.Nx), dtype=torch.float32, device=dev)
+    ts = time_propagation(bb, w, dev, field0, dn, nref, inten, flags=flags, runs=runs, scratch=scratch)
+    med, mn = statistics.median(ts), min(ts)
+    units = float(w.Nx) * w.Ny * w.Nz * B
+    out = {"workload": "%s%s: %d field(s) of %dx%d, %d z-slices%s" % (w.name, " per-field intensity" if per_field else "", B, w.Nx, w.Ny, w.Nz,
+                                                                     ", %.1f GiB intensity out" % (inten.numel() * 4 / 2**30) if per_field else ""),
+           "baseline_config": "BASELINE.json configs[%d]" % w.index,
+           "propagate_ms": med, "propagate_ms_min": mn, "runs": len(ts),
+           "value": units / (med * 1e-3) / 1e6, "unit": "Mvox/s", "kernel": bb.last_kernel(),
+           "roofline": roofline_fracs(w, med * 1e-3, peaks, per_field)}
+    del inten, dn
+    return out
+
+
 def run_ours(args):
     from paper_1706_02261_b200 import binding as bb, build
     rank, local_rank, _ = replicas.env_world()
     world = replicas.init()
+    if world != args.gpus:
+        raise SystemExit("bench.py --gpus %d runs under a world of %d ranks: launch it with torchrun --nproc-per-node %d "
+                         "(or let `python bench.py --gpus N` start the ranks itself)" % (args.gpus, world, args.gpus))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
     dev = torch.device("cuda", local_rank if world > 1 else 0)
@@ -150,7 +228,6 @@ def run_ours(args):
     B, npx = w.batch, w.Nx * w.Ny
     flags = bb.LAUNCH_PER_PHASE if args.per_phase else 0
     dn, f0, em = make_inputs(w, dev)
-    nref = bb.nref_from_dn(dn, w.n0, w.nref_slab).numpy()
     if em is not None:
         em_d = tuple(t.to(dev) for t in em)
         field = torch.empty((1, w.Ny, w.Nx), dtype=torch.complex64, device=dev)
@@ -160,7 +237,7 @@ def run_ours(args):
     inten = torch.empty((w.Nz, w.Ny, w.Nx), dtype=torch.float32, device=dev)
     ev = lambda: torch.cuda.Event(enable_timing=True)
 
-    def step(marks=None):
+    def step(marks=None, nref=None):
         if em is not None:
             bb.multiplex_psf(em_d[0], em_d[1], em_d[2], w.NA, w.Nx, w.Ny, w.dx, w.lam, out=field[0])
         else:
@@ -172,8 +249,17 @@ def run_ours(args):
             b = ev(); b.record()
             marks.append((a, b))
 
+    # cold: the first pass of the hot path in this process -- plan, twiddle and propagator tables,
+    # the n_ref helper (one pass over dn) and the propagation itself (SURVEY 8d "reported additionally cold")
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    nref = bb.nref_from_dn(dn, w.n0, w.nref_slab).numpy()
+    step(nref=nref)
+    torch.cuda.synchronize()
+    cold_ms = (time.perf_counter() - t0) * 1e3
+
     for _ in range(args.warmup):
-        step()
+        step(nref=nref)
     torch.cuda.synchronize()
     bb.device_status()
     replicas.barrier()
@@ -184,7 +270,7 @@ def run_ours(args):
     torch.cuda.synchronize()
     e0.record()
     for _ in range(args.steps):
-        step(marks)
+        step(marks, nref=nref)
     e1.record()
     torch.cuda.synchronize()
     replicas.barrier()
@@ -195,7 +281,9 @@ def run_ours(args):
     t = replicas.max_over_ranks(t_local)
     units = float(npx) * w.Nz * B * args.steps                 # pixel-slices this rank processed
     value = replicas.sum_over_ranks(units) / t / 1e6
-    prop_ms = statistics.mean(a.elapsed_time(b) for a, b in marks)   # the propagate call = the BPM kernel(s)
+    prop_all = [a.elapsed_time(b) for a, b in marks]           # the propagate call = the BPM kernel(s)
+    prop_ms = statistics.mean(prop_all)
+    kernel_name = bb.last_kernel()
 
     result = {
         "metric": "pixel-slices per second through the split-step BPM (ms per full propagation = ms_per_step)",
@@ -214,7 +302,8 @@ def run_ours(args):
                    "launch_mode": "per-phase kernels" if args.per_phase else "one persistent cooperative kernel per propagation",
                    "headline": bool(args.workload == "C4" and not args.nz)},
         "gpu_launches": int(launches),
-        "propagate_ms": prop_ms,
+        "propagate_ms": prop_ms, "propagate_ms_median": statistics.median(prop_all), "propagate_ms_min": min(prop_all),
+        "cold_ms": cold_ms,
     }
     if clocks is not None:
         result["clocks"] = clocks
@@ -222,12 +311,15 @@ def run_ours(args):
     # ---- roofline of the dominant kernel (the persistent BPM kernel, one launch per propagation) ----
     hbm_b, l2_b, flop = algorithmic_per_step(w)
     hbm_peak, hbm_src = measured_peaks()
+    peaks = {"hbm": hbm_peak}
     dur = prop_ms * 1e-3
     traffic = committed_dram_traffic(w.name if (not args.nz and B == 1) else "")
+    traffic_note = ("ncu capture of this source digest (profiles/dram_traffic.csv)" if traffic is not None
+                    else "null: no ncu capture of the library source being timed (profiles/dram_traffic.csv holds other digests)")
     alu_ach = flop * w.Nz / dur / 1e12
     result["roofline"] = {"bound": "alu", "achieved": alu_ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
-                          "frac": alu_ach / FP32_PEAK_TFLOPS, "traffic": traffic,
-                          "kernel": "bb::bpm16_kernel<4,4,4,false>" if (w.Nx, w.Ny, B) == (1024, 1024, 1) else "bb::bpm_kernel / bb::bpm16_kernel", "peak_source": "nominal 148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md)",
+                          "frac": alu_ach / FP32_PEAK_TFLOPS, "traffic": traffic, "traffic_source": traffic_note,
+                          "kernel": kernel_name, "peak_source": "nominal 148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md)",
                           "algorithmic_flop_per_launch": flop * w.Nz}
     hbm_ach = hbm_b * w.Nz / dur / 1e9
     result["roofline_hbm"] = {"bound": "hbm", "achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s",
@@ -235,25 +327,21 @@ def run_ours(args):
                               "algorithmic_bytes_per_launch": hbm_b * w.Nz}
     if rank == 0 and not args.no_probe:
         try:
-            l2_peak = bb.probe_l2_bandwidth(32 << 20, 200, 0)
+            peaks["l2_copy"] = bb.probe_l2_bandwidth(32 << 20, 200, 0)
+            peaks["l2_read"] = bb.probe_l2_bandwidth(32 << 20, 200, 1)
             fp32_meas = bb.probe_fp32(20000, False)
             l2_ach = l2_b * w.Nz / dur / 1e9
-            result["roofline_l2"] = {"bound": "l2", "achieved": l2_ach, "peak": l2_peak, "unit": "GB/s",
-                                     "frac": l2_ach / l2_peak,
-                                     "peak_source": "measured now: bb_probe_l2_bandwidth, 32 MiB resident copy",
+            result["roofline_l2"] = {"bound": "l2", "achieved": l2_ach, "peak": peaks["l2_copy"], "unit": "GB/s",
+                                     "frac": l2_ach / peaks["l2_copy"],
+                                     "peak_read_only": peaks["l2_read"], "frac_vs_read_peak": l2_ach / peaks["l2_read"],
+                                     "peak_source": "measured now: bb_probe_l2_bandwidth, 32 MiB resident, copy (half read, half "
+                                                    "write, like the field's traffic) and read-only",
                                      "algorithmic_bytes_per_launch": l2_b * w.Nz}
             result["roofline"]["peak_measured_fma_loop"] = fp32_meas
-            t_roof = max(hbm_b / (hbm_peak * 1e9), l2_b / (l2_peak * 1e9))
+            t_roof = max(hbm_b / (hbm_peak * 1e9), l2_b / (peaks["l2_copy"] * 1e9))
             result["hbm_l2_roofline_frac"] = t_roof / (dur / w.Nz)       # T_roof / T_measured per slice
         except Exception as e:                                            # noqa: BLE001
             result["roofline_l2"] = {"error": str(e)}
-
-    # ---- the batched workload (BASELINE.json configs[4]) beside the headline, for information ----
-    if rank == 0 and world == 1 and args.workload == "C4" and not args.nz and not args.no_batch:
-        try:
-            result["batch_workload"] = time_batch_workload(bb, dev)
-        except Exception as e:                                            # noqa: BLE001
-            result["batch_workload"] = {"error": str(e)}
 
     # ---- end to end through the host-buffer entry point ----
     if not args.no_e2e:
@@ -299,33 +387,29 @@ def run_ours(args):
     # ---- the oracle on this box's host cores (reported baseline, rank 0, N = 1 only) ----
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         result["cpu_baseline"] = oracle_sample(w, dn, f0, em, nref, budget_s=args.cpu_seconds)
+        try:
+            result["cpu_baseline"]["one_thread"] = oracle_sample(w, dn, f0, em, nref, budget_s=args.cpu_seconds / 2, threads=1)
+        except Exception as e:                                            # noqa: BLE001
+            result["cpu_baseline"]["one_thread"] = {"error": str(e)}
+
+    # ---- the other configurations of BASELINE.json (parity-test cases), timed for information ----
+    if rank == 0 and world == 1 and args.workload == "C4" and not args.nz and not args.no_configs:
+        del dn, inten
+        torch.cuda.empty_cache()
+        scratch = torch.zeros(64 << 20, dtype=torch.float32, device=dev)          # 256 MiB
+        cfgs = []
+        for name, per_field in (("C1", False), ("C2", False), ("C3", False), ("C5", False), ("C5", True)):
+            try:
+                cfgs.append(time_config(bb, dev, name, peaks, scratch, per_field=per_field))
+            except Exception as e:                                        # noqa: BLE001
+                cfgs.append({"workload": name, "error": str(e)})
+        result["configs"] = cfgs
+        result["configs_note"] = ("3 warm-ups, median (propagate_ms) and min of 10 propagations each, 256 MiB written between runs; "
+                                  "C1-C3 are latency-bound (T_roof is sub-microsecond per step): their fractions are for information")
 
     if rank == 0:
         print(json.dumps(result))
     replicas.shutdown()
-
-
-def time_batch_workload(bb, dev, steps=3):
-    """C5: 16 fields of 512x512 through a shared 512^3 volume, summed intensity (device-resident)."""
-    w = wl.config("C5")
-    dn, f0, _ = make_inputs(w, dev)
-    nref = bb.nref_from_dn(dn, w.n0, w.nref_slab).numpy()
-    f0_d = torch.from_numpy(f0).to(dev)
-    field = torch.empty_like(f0_d)
-    inten = torch.empty((w.Nz, w.Ny, w.Nx), dtype=torch.float32, device=dev)
-    ts = []
-    for i in range(steps + 2):
-        field.copy_(f0_d)
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record()
-        bb.propagate(field, dn, w.dx, w.dz, w.lam, w.n0, intensity=inten, nref=nref)
-        b.record()
-        torch.cuda.synchronize()
-        if i >= 2:
-            ts.append(a.elapsed_time(b))
-    ms = statistics.mean(ts)
-    return {"workload": "C5: %d fields of %dx%d, %d z-slices, one shared dn volume, summed intensity" % (w.batch, w.Nx, w.Ny, w.Nz),
-            "propagate_ms": ms, "value": w.batch * w.Nx * w.Ny * w.Nz / (ms * 1e-3) / 1e6, "unit": "Mvox/s"}
 
 
 def run_trace(args):
@@ -371,10 +455,22 @@ def run_trace(args):
     print(json.dumps(out))
 
 
-def oracle_sample(w, dn, f0, em, nref, budget_s=15.0, slices=None):
-    """Times the oracle, as it stands, on the first `slices` z-slices of the workload."""
+def oracle_sample(w, dn, f0, em, nref, budget_s=15.0, slices=None, threads=None):
+    """Times the oracle, as it stands, on the first `slices` z-slices of the workload (threads: OpenMP
+    thread count for this sample, None = all cores of the affinity mask)."""
+    import ctypes
     import oracle
     oracle.build()
+    ncores = oracle.num_threads()
+    if threads is not None:
+        gomp = ctypes.CDLL("libgomp.so.1")
+        gomp.omp_set_num_threads(int(threads))
+        try:
+            r = oracle_sample(w, dn, f0, em, nref, budget_s=budget_s, slices=slices)
+        finally:
+            gomp.omp_set_num_threads(ncores)
+        r["cores"] = int(threads)
+        return r
     if f0 is None:
         pos, ph, amp = (t.numpy() for t in em)
         u0 = oracle.multiplex_psf(pos, ph, amp, w.NA, w.Nx, w.Ny, w.dx, w.lam).astype(np.complex64)
@@ -451,7 +547,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-probe", action="store_true")
-    ap.add_argument("--no-batch", action="store_true", help="skip the C5 batched-fields timing")
+    ap.add_argument("--no-batch", "--no-configs", dest="no_configs", action="store_true",
+                    help="skip the timing of the other BASELINE.json configurations (C1-C3, C5 summed and per-field)")
     ap.add_argument("--trace", type=int, default=0, metavar="N",
                     help="print the per-phase timeline of the persistent kernel over the first N z-steps and exit")
     ap.add_argument("--e2e-steps", type=int, default=3)
@@ -459,6 +556,14 @@ def main():
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours" and not args.nz:
         args.warmup = 3                                   # timing rule: at least 3 warm-up steps
+    if args.impl == "ours" and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # `python bench.py --gpus N` without a launcher: start the N ranks ourselves (one process per GPU)
+        import socket
+        with socket.socket() as so:
+            so.bind(("127.0.0.1", 0))
+            port = so.getsockname()[1]
+        os.execvp(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+                                   "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:])
     if args.trace:
         run_trace(args)
     elif args.impl == "reference":

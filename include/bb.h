@@ -211,6 +211,7 @@ const char *bb_last_error(void);        /* thread-local; "" if none */
 int bb_version(void);                   /* 100 * major + minor */
 void bb_shutdown(void);                 /* frees cached plans, tables and workspace (synchronises) */
 unsigned long long bb_launch_count(void); /* kernels launched by this library since load */
+const char *bb_last_kernel(void);        /* name of the BPM kernel the last propagation launched ("" if none yet) */
 int bb_device_status(void);             /* synchronises the device; BB_ERR_INTERNAL if a device-side
                                            watchdog tripped since the last call, else BB_OK */
 

@@ -24,7 +24,7 @@ HOMOGENEOUS = 16
 EXPORTS = ("bb_propagate", "bb_propagate_ex", "bb_propagate_host", "bb_nref_from_dn",
            "bb_multiplex_psf", "bb_fft2", "bb_propagator_table", "bb_last_error", "bb_version",
            "bb_shutdown", "bb_launch_count", "bb_device_status", "bb_probe_l2_bandwidth", "bb_probe_fp32", "bb_probe_trace",
-           "bb_multiplex_annular", "bb_lightsheet", "bb_refocus", "bb_extract_tiles", "bb_image_formation")
+           "bb_last_kernel", "bb_multiplex_annular", "bb_lightsheet", "bb_refocus", "bb_extract_tiles", "bb_image_formation")
 
 STATUS_NAMES = {0: "BB_OK", 1: "BB_ERR_INVALID_ARG", 2: "BB_ERR_UNSUPPORTED_SHAPE", 3: "BB_ERR_CUDA",
                 4: "BB_ERR_OOM", 5: "BB_ERR_ARCH", 6: "BB_ERR_INTERNAL"}
@@ -72,6 +72,7 @@ def load() -> ctypes.CDLL:
     lib.bb_probe_fp32.argtypes = [i, i, ctypes.POINTER(ctypes.c_double)]
     lib.bb_probe_trace.argtypes = [ctypes.c_void_p, i]
     lib.bb_last_error.restype = ctypes.c_char_p
+    lib.bb_last_kernel.restype = ctypes.c_char_p
     lib.bb_launch_count.restype = ctypes.c_ulonglong
     lib.bb_shutdown.restype = None
     _lib = lib
@@ -287,6 +288,10 @@ def probe_fp32(iters: int = 20000, packed: bool = False) -> float:
 
 def device_status():
     _check(load().bb_device_status())
+
+
+def last_kernel() -> str:
+    return load().bb_last_kernel().decode()
 
 
 def launch_count() -> int:

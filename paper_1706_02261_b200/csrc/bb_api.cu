@@ -26,6 +26,7 @@ unsigned long long g_launches = 0;
 long long *g_trace = nullptr;      // bb_probe_trace
 int g_trace_phases = 0;
 int g_trace_dev = -1;
+char g_last_kernel[96] = "";      // bb_last_kernel
 
 int fail(int code, const char *fmt, ...) {
     char buf[512];
@@ -422,6 +423,9 @@ int launch_steps(Plan *p, cf *field, const float *dn, float *inten, long long in
     if (!k8 && !k16 && !p->k32) return fail(BB_ERR_UNSUPPORTED_SHAPE, "no kernel for Nx = %d, Ny = %d, batch = %d", p->Nx, p->Ny, B);
     if (k16 || k8) P.use_tma = make_field_tmap(&P.tmap, field, p->Nx, p->Ny, B, p->cw4 ? 4 : 8) ? 1 : 0;
     if (g_trace && g_trace_dev == p->device && (k16 || k8) && 2 * Nz_total + 1 <= g_trace_phases) { P.trace = g_trace; P.trace_p0 = 0; }
+    snprintf(g_last_kernel, sizeof g_last_kernel, k8 ? "bb::bpm8_kernel<%d,%d,%d,%s>" : k16 ? "bb::bpm16_kernel<%d,%d,%d,%s>" : "bb::bpm_kernel<%d,%d,%d>",
+             k8 || k16 ? p->Nx / 256 : p->Nx / 32, k8 || k16 ? p->Ny / 256 : p->Ny / 32, k8 || k16 ? (p->cw4 ? 4 : 8) : 8,
+             B > 1 ? "true" : "false");
     auto launch = [&](bool coop) {
         return k8 ? bb::kernel8_launch(p->Nx, p->Ny, P, p->grid, coop, s)
                   : k16 ? bb::kernel16_launch(p->Nx, p->Ny, P, p->grid, coop, s)
@@ -629,6 +633,7 @@ cudaError_t kernel8_launch(int Nx, int Ny, const KParams &P, int grid, bool coop
 extern "C" {
 
 const char *bb_last_error(void) { return g_err.c_str(); }
+const char *bb_last_kernel(void) { return g_last_kernel; }
 int bb_version(void) { return 100; }
 unsigned long long bb_launch_count(void) { return g_launches; }
 
