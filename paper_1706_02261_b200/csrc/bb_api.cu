@@ -89,6 +89,14 @@ struct Plan {
     unsigned long long tick = 0;
 };
 
+void destroy_plan(Plan *p) {
+    for (void *q : {(void *)p->twx, (void *)p->twy, (void *)p->tw256, (void *)p->twcx, (void *)p->twcy, (void *)p->bar,
+                    (void *)p->status, (void *)p->d_htab, (void *)p->d_phase, (void *)p->d_fmax})
+        if (q) cudaFree(q);
+    for (TableEntry &e : p->tables) cudaFree(e.ptr);
+    delete p;
+}
+
 std::vector<Plan *> g_plans;
 struct Workspace { void *ptr = nullptr; size_t bytes = 0; };
 // Everything the library allocates outside a plan belongs to ONE device: workspaces of the host-buffer
@@ -145,6 +153,7 @@ int get_plan(int Nx, int Ny, Plan **out) {
     for (Plan *p : g_plans)
         if (p->device == dev && p->Nx == Nx && p->Ny == Ny) { *out = p; return BB_OK; }
     Plan *p = new Plan();
+    struct Guard { Plan *p; ~Guard() { if (p) destroy_plan(p); } } guard{p};   // every early return releases what was allocated
     p->device = dev; p->Nx = Nx; p->Ny = Ny; p->sm_count = sms;
     if (Nx <= 1024 && Ny <= 1024) {
         std::vector<cf> tx = make_twiddles(Nx), ty = make_twiddles(Ny);
@@ -186,14 +195,14 @@ int get_plan(int Nx, int Ny, Plan **out) {
         BB_CUDA(cudaMemcpy(p->twcy, cy.data(), cy.size() * sizeof(cf), cudaMemcpyHostToDevice));
         if (want16) {
             int rc16 = bb::kernel16_prepare(Nx, Ny);
-            if (rc16 != 0) { delete p; return fail(BB_ERR_CUDA, "kernel16_prepare failed: %s", cudaGetErrorString((cudaError_t)rc16)); }
-            if (bb::kernel16_blocks_per_sm(Nx, Ny) < 1) { delete p; return fail(BB_ERR_CUDA, "16-point BPM kernel does not fit on an SM"); }
+            if (rc16 != 0) { return fail(BB_ERR_CUDA, "kernel16_prepare failed: %s", cudaGetErrorString((cudaError_t)rc16)); }
+            if (bb::kernel16_blocks_per_sm(Nx, Ny) < 1) { return fail(BB_ERR_CUDA, "16-point BPM kernel does not fit on an SM"); }
             p->k16 = true;
         }
         if (want8) {
             int rc8 = bb::kernel8_prepare(Nx, Ny);
-            if (rc8 != 0) { delete p; return fail(BB_ERR_CUDA, "kernel8_prepare failed: %s", cudaGetErrorString((cudaError_t)rc8)); }
-            if (bb::kernel8_blocks_per_sm(Nx, Ny) < 1) { delete p; return fail(BB_ERR_CUDA, "8-point BPM kernel does not fit on an SM"); }
+            if (rc8 != 0) { return fail(BB_ERR_CUDA, "kernel8_prepare failed: %s", cudaGetErrorString((cudaError_t)rc8)); }
+            if (bb::kernel8_blocks_per_sm(Nx, Ny) < 1) { return fail(BB_ERR_CUDA, "8-point BPM kernel does not fit on an SM"); }
             p->k8 = true;
             p->force_k8 = getenv("BB_USE_K8") != nullptr;
         }
@@ -202,13 +211,14 @@ int get_plan(int Nx, int Ny, Plan **out) {
     p->table_capacity = std::max<size_t>(2, std::min<size_t>(4096, table_budget_bytes() / tb));
     if (Nx <= 1024 && Ny <= 1024) {
         rc = bb::kernel_prepare(Nx, Ny);
-        if (rc != 0) { delete p; return fail(BB_ERR_CUDA, "kernel_prepare failed: %s", cudaGetErrorString((cudaError_t)rc)); }
+        if (rc != 0) { return fail(BB_ERR_CUDA, "kernel_prepare failed: %s", cudaGetErrorString((cudaError_t)rc)); }
         int per_sm = bb::kernel_blocks_per_sm(Nx, Ny);
-        if (per_sm < 1) { delete p; return fail(BB_ERR_CUDA, "BPM kernel does not fit on an SM"); }
+        if (per_sm < 1) { return fail(BB_ERR_CUDA, "BPM kernel does not fit on an SM"); }
         p->k32 = true;
     }
-    if (!p->k32 && !p->k8) { delete p; return fail(BB_ERR_UNSUPPORTED_SHAPE, "no kernel for Nx = %d, Ny = %d", Nx, Ny); }
+    if (!p->k32 && !p->k8) { return fail(BB_ERR_UNSUPPORTED_SHAPE, "no kernel for Nx = %d, Ny = %d", Nx, Ny); }
     p->grid = sms;
+    guard.p = nullptr;
     g_plans.push_back(p);
     *out = p;
     return BB_OK;
@@ -297,10 +307,11 @@ int get_table(Plan *p, const TableKey &k, cudaStream_t s, unsigned long long pro
             if (e.last_use < protect_tick && (!slot || e.last_use < slot->last_use)) slot = &e;
         if (!slot) return kTableCacheFull;
     }
-    slot->key = k;
-    slot->last_use = p->tick;
+    slot->key = TableKey{0.f, 0.f, 0.f, -1.f, 0};            // no table until the build has been enqueued
     int rc = build_table(p, k, slot->ptr, s);
     if (rc) return rc;
+    slot->key = k;
+    slot->last_use = p->tick;
     *out = slot->ptr;
     return BB_OK;
 }
@@ -640,15 +651,7 @@ unsigned long long bb_launch_count(void) { return g_launches; }
 void bb_shutdown(void) {
     std::lock_guard<std::mutex> lk(g_mu);
     cudaDeviceSynchronize();
-    for (Plan *p : g_plans) {
-        cudaFree(p->twx); cudaFree(p->twy); cudaFree(p->bar); cudaFree(p->status);
-        if (p->tw256) { cudaFree(p->tw256); cudaFree(p->twcx); cudaFree(p->twcy); }
-        for (TableEntry &e : p->tables) cudaFree(e.ptr);
-        if (p->d_htab) cudaFree((void *)p->d_htab);
-        if (p->d_phase) cudaFree(p->d_phase);
-        if (p->d_fmax) cudaFree(p->d_fmax);
-        delete p;
-    }
+    for (Plan *p : g_plans) destroy_plan(p);
     g_plans.clear();
     for (auto &kv : g_ctx) {
         DeviceCtx &c = kv.second;

@@ -457,12 +457,17 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
                 cf *stage = sm_y + tm.team * (TM::TEAM * 17);
                 unsigned long long *bar = sm_mbar + tm.team;
                 if (threadIdx.x % TM::TEAM == 0) {
-                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    // the tile was written by other CTAs through the generic proxy (st.global) and the landing
+                    // zone by this CTA: order both before the async-proxy copy
+                    asm volatile("fence.proxy.async;" ::: "memory");
                     mbar_expect_tx(bar, (unsigned)(P * kL * CW * sizeof(cf)));
 #pragma unroll
                     for (int cc = 0; cc < P; ++cc) tma_load_4d(stage + cc * kL * CW, &K.tmap, u * CW, cc, 0, b, bar);
                 }
-                if (!mbar_wait(bar, uc.tma_parity)) atomicExch(K.status, 2);
+                if (!mbar_wait(bar, uc.tma_parity)) {       // the copy never arrived: flag it and leave the phase; the grid
+                    atomicExch(K.status, 2);                // barrier's watchdog sees the flag and ends the kernel
+                    return;
+                }
                 uc.tma_parity ^= 1u;
 #pragma unroll
                 for (int i = 0; i < 16; ++i) v[i] = stage[(tm.c * kL + tm.t + 16 * i) * CW + tm.col];

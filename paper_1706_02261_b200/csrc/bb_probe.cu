@@ -70,7 +70,8 @@ int bb_probe_l2_bandwidth(unsigned long long bytes, int iters, int mode, double 
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     void *buf = nullptr;
     float *sink = nullptr;
-    if (cudaMalloc(&buf, bytes) != cudaSuccess || cudaMalloc(&sink, 256) != cudaSuccess) return BB_ERR_OOM;
+    if (cudaMalloc(&buf, bytes) != cudaSuccess) return BB_ERR_OOM;
+    if (cudaMalloc(&sink, 256) != cudaSuccess) { cudaFree(buf); return BB_ERR_OOM; }
     cudaMemset(buf, 0, bytes);
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0);

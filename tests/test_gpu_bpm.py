@@ -291,6 +291,15 @@ def _full_config_parity(bb, oracle, name, nz=None, batch_limit=None):
     print("\n%s: Nz=%d B=%d  field rel-L2 %.3e  intensity rel-L2 %.3e  (per-slice intensity error: "
           "first %.2e, mid %.2e, last %.2e)" % (name, w.Nz, B, err_u, cmp_I.rel, cmp_I.curve[0],
                                                cmp_I.curve[len(cmp_I.curve) // 2], cmp_I.curve[-1]))
+    # SURVEY 8c-R1 "the slope is the real check": the field error of an fp32 transform pair grows linearly at
+    # ~5e-8 per step and the intensity error of a slice is ~2x the field error there, so a least-squares line
+    # through (per-slice intensity error) / 2 must not be steeper than 6e-8 per step (single fields only: the
+    # summed intensity of a batch averages the errors of its fields)
+    if B == 1 and w.Nz >= 64:
+        j = np.arange(1, w.Nz + 1, dtype=np.float64)
+        slope = float(np.sum(j * (np.array(cmp_I.curve) / 2)) / np.sum(j * j))       # line through the origin
+        print("%s: per-step growth of the field error, from the intensity curve: %.2e" % (name, slope))
+        assert slope <= 6e-8, slope
     return err_u, cmp_I.rel
 
 
@@ -300,6 +309,45 @@ def test_config_parity_full(oracle_mod, name):
     bb = need_gpu()
     err_u, err_I = _full_config_parity(bb, oracle_mod, name)
     assert err_u < TOL and err_I < TOL
+
+
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C5"])
+def test_no_mode_sits_on_the_evanescent_cut(name):
+    """a mode with |s| < 1e-9 k^2 could be classified either way; the harness asserts that no such
+    mode exists for any reference index the measured configurations use (n_ref slabs of 32 slices), so the
+    result is unique.  s = k^2 - kx^2 - ky^2 in double from the float32 scalars, as both sides compute it."""
+    bb = need_gpu()
+    w = wl.config(name)
+    dn = wl.make_dn(w, device="cuda").cuda()
+    nref = bb.nref_from_dn(dn, w.n0, w.nref_slab).numpy()
+    del dn
+    f32 = lambda x: float(np.float32(x))
+    kx = 2 * np.pi * np.fft.fftfreq(w.Nx, d=f32(w.dx))
+    ky = 2 * np.pi * np.fft.fftfreq(w.Ny, d=f32(w.dx))
+    k2 = (kx * kx)[None, :] + (ky * ky)[:, None]
+    for nr in np.unique(np.concatenate([nref, np.array([w.n0], dtype=np.float32)])):
+        k = 2 * np.pi / f32(w.lam) * float(nr)
+        margin = float(np.abs(k * k - k2).min() / (k * k))
+        assert margin > 1e-9, (name, float(nr), margin)
+
+
+def test_config_c5_per_field_intensity_parity(oracle_mod):
+    """configs[4] with BB_INTENSITY_PER_FIELD ("C5 is measured both summed and per-field"): 16 volumes,
+    24 of the 512 slices, every element against the oracle's 16 runs."""
+    bb = need_gpu()
+    w = wl.config("C5").with_nz(24)
+    dn, f_gpu = gpu_inputs(w, bb)
+    f0 = oracle_field0(w, oracle_mod)
+    nref = bb.nref_from_dn(dn, w.n0, w.nref_slab).numpy()
+    I = torch.full((w.batch, w.Nz, w.Ny, w.Nx), float("nan"), device="cuda")
+    bb.propagate(f_gpu, dn, w.dx, w.dz, w.lam, w.n0, intensity=I, nref=nref, flags=bb.INTENSITY_PER_FIELD)
+    torch.cuda.synchronize()
+    bb.device_status()
+    dn_h = dn.cpu().numpy()
+    for b in range(w.batch):
+        uo, Io = oracle_mod.propagate(f0[b], dn_h, w.dx, w.dz, w.lam, w.n0, nref=nref)
+        assert rel_l2(f_gpu[b].cpu().numpy(), uo) < TOL
+        assert rel_l2(I[b].cpu().numpy(), Io) < TOL
 
 
 def test_config_c5_batched_parity(oracle_mod):
