@@ -218,6 +218,7 @@ int get_plan(int Nx, int Ny, Plan **out) {
     }
     if (!p->k32 && !p->k8) { return fail(BB_ERR_UNSUPPORTED_SHAPE, "no kernel for Nx = %d, Ny = %d", Nx, Ny); }
     p->grid = sms;
+    if (getenv("BB_GRID")) p->grid = std::max(1, std::min(sms, atoi(getenv("BB_GRID"))));   // diagnostic: persistent grid size
     guard.p = nullptr;
     g_plans.push_back(p);
     *out = p;

@@ -70,15 +70,10 @@ struct KParams {
 // phase r the propagator of step r.  Backward (time reversal, Fig. 2c): a step is "x conj screen,
 // FFT2, x conj H, IFFT2", so row phase r applies the screen of step Nz - 1 - r (r < Nz) BEFORE the
 // transform pair that column phase r completes with the table of the same step.
-#ifdef BB_FWD_ONLY
-__device__ __forceinline__ int row_step(const KParams &P, int r) { return r - 1; }
-__device__ __forceinline__ int col_step(const KParams &P, int r) { return r; }
-#else
 __device__ __forceinline__ int row_step(const KParams &P, int r) {
     return P.backward ? (r < P.Nz_total ? P.Nz_total - 1 - r : -1) : r - 1;
 }
 __device__ __forceinline__ int col_step(const KParams &P, int r) { return P.backward ? P.Nz_total - 1 - r : r; }
-#endif
 
 __device__ __forceinline__ cf ld_cg(const cf *p) { return __ldcg(p); }
 __device__ __forceinline__ void st_cg(cf *p, cf v) { __stcg(p, v); }

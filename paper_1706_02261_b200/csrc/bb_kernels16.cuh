@@ -690,11 +690,7 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const __grid_const
             run_phase16<PX, 1, true, NX, NY, BATCH>(P, d, sm_tw, sm_twcx, sm_y, sm_pwS, tagS, ucR, Fa, CWC);
         } else {
             run_phase16<PY, CWC, false, NX, NY, BATCH>(P, d, sm_tw, sm_twcy, sm_y, sm_pwH, tagH, ucC, Fa, CWC, sm_mbar,
-#ifdef BB_NO_IDLE_STAGING
-                                                       -1, sm_pwS, &tagS);
-#else
                                                        (!BATCH && p + 1 < P.p1) ? p + 1 : -1, sm_pwS, &tagS);
-#endif
         }
         if (tracer) tr[1] = clock64();
         if (BATCH && d.is_row && d.kind == 1 && P.inten != nullptr && !(P.flags & 2u) && P.B > 1)
@@ -715,11 +711,7 @@ __global__ void __launch_bounds__(kThreads16, 1) bpm16_kernel(const __grid_const
                 prefill_phase16<PY, CWC, false, NX, NY, BATCH>(P, d_next, sm_pwH, tagH, Fn);
                 // screen factors of the row phase after next: here, unless the coming column phase has
                 // idle warps for them (same live band as the last column phase, which had an idle team)
-#ifdef BB_NO_IDLE_STAGING
-                const bool col_stages = false;
-#else
                 const bool col_stages = !BATCH && ucC.F == Fn && (ucC.a1 - ucC.a0) < Team16<PY, CWC>::NTEAM;
-#endif
                 if (p + 2 < P.p1 && !col_stages) prefill_phase16<PX, 1, true, NX, NY, BATCH>(P, decode_phase16(P, p + 2), sm_pwS, tagS, 0);
             } else {
                 prefill_phase16<PX, 1, true, NX, NY, BATCH>(P, d_next, sm_pwS, tagS, 0);
