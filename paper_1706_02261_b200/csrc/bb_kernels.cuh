@@ -399,6 +399,8 @@ __device__ __forceinline__ void grid_arrive(unsigned *bar) {
     if (threadIdx.x == 0)
         asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(bar) : "memory");
 }
+// (measured alternatives, both slower on an empty phase loop, 1.55 us per barrier as written: polling with
+// relaxed loads plus one acquire fence 1.75 us; every thread fencing its own stores and a relaxed add 1.87 us)
 __device__ __forceinline__ bool grid_wait(unsigned *bar, unsigned target, int *status, int *sm_abort) {
     if (threadIdx.x == 0) {
         unsigned spins = 0;

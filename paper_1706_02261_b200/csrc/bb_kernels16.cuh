@@ -333,25 +333,44 @@ __device__ __forceinline__ void stage_screen_by_idle_warps(const KParams &K, con
 #pragma unroll
             for (int k = 0; k < PER; ++k)
                 x[rl][k] = (rb + rl < rows && s + k * TEAMC < NX && !K.noscreen) ? __ldcs(dnp + (rb + rl) * NX + k * TEAMC) : 0.f;
+        // ONE decision for the whole chunk (small arguments: the compact packed path), so that the code
+        // the warp walks through stays short: a vote and both paths per value made the staging
+        // instruction-fetch bound (5 us for 28 values per thread)
+        float amax = 0.f;
 #pragma unroll
-        for (int rl = 0; rl < RCH; ++rl) {
-            if (rb + rl < rows) {
+        for (int rl = 0; rl < RCH; ++rl)
 #pragma unroll
-                for (int k = 0; k < PER; ++k) {
-                    const int n = s + k * TEAMC;
-                    if (n < NX) {
-                        const int m = n >> 8, q = n & 255, t = q & 15, z = q >> 4, c = z % PX, jp = z / PX;
-                        const float a = fmaf(pb, x[rl][k], pa);
-                        cf f;
-                        if (__all_sync(__activemask(), fabsf(a) <= 0.78539816f)) {
-                            f = screen_cossin_small_packed(a);
-                        } else {
-                            float sn, cs;
-                            screen_sincos(a, sn, cs);
-                            f = make_float2(cs, sn);
+            for (int k = 0; k < PER; ++k) {
+                x[rl][k] = fmaf(pb, x[rl][k], pa);
+                amax = fmaxf(amax, fabsf(x[rl][k]));
+            }
+        const bool small = __all_sync(__activemask(), amax <= 0.78539816f);
+        if (small) {
+#pragma unroll
+            for (int rl = 0; rl < RCH; ++rl) {
+                if (rb + rl < rows) {
+#pragma unroll
+                    for (int k = 0; k < PER; ++k) {
+                        const int n = s + k * TEAMC;
+                        if (n < NX) {
+                            const int m = n >> 8, q = n & 255, t = q & 15, z = q >> 4, c = z % PX, jp = z / PX;
+                            sm_pwS[(jp * PX + m) * kThreads16 + (rb + rl) * TR::TEAM + c * 16 + t] = screen_cossin_small_packed(x[rl][k]);
                         }
-                        sm_pwS[(jp * PX + m) * kThreads16 + (rb + rl) * TR::TEAM + c * 16 + t] = f;
                     }
+                }
+            }
+        } else {
+#pragma unroll 1
+            for (int i = 0; i < RCH * PER; ++i) {
+                const int rl = i / PER, k = i % PER, n = s + k * TEAMC;
+                if (rb + rl < rows && n < NX) {
+                    const int m = n >> 8, q = n & 255, t = q & 15, z = q >> 4, c = z % PX, jp = z / PX;
+                    float sn, cs;
+                    float a = 0.f;
+#pragma unroll
+                    for (int u = 0; u < RCH * PER; ++u) a = (u == i) ? x[u / PER][u % PER] : a;     // registers, not a local array
+                    screen_sincos(a, sn, cs);
+                    sm_pwS[(jp * PX + m) * kThreads16 + (rb + rl) * TR::TEAM + c * 16 + t] = make_float2(cs, sn);
                 }
             }
         }
@@ -374,6 +393,22 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
     constexpr long long CS = ROW ? kL : NX;              // class stride: class-major (rows) / interleaved (columns)
     constexpr long long IS = ROW ? 1 : (long long)P * NX;   // stride inside a class
     const TM tm;
+    // Column phase of a single field: the tile request goes out before anything else is computed (the
+    // team's first tile is known from the previous step unless the live band changed): the L2 -> shared
+    // memory copy is ~1 us of pure latency at the head of the phase.
+    bool tma_issued = false;
+    if constexpr (!ROW && !BATCH) {
+        if (K.use_tma && uc.F == Fin && uc.a0 + tm.team < uc.a1) {
+            if (threadIdx.x % TM::TEAM == 0) {
+                cf *stage0 = sm_y + tm.team * (TM::TEAM * 17);
+                asm volatile("fence.proxy.async;" ::: "memory");
+                mbar_expect_tx(sm_mbar + tm.team, (unsigned)(P * kL * CW * sizeof(cf)));
+#pragma unroll
+                for (int cc = 0; cc < P; ++cc) tma_load_4d(stage0 + cc * kL * CW, &K.tmap, uc.u0 * CW, cc, 0, 0, sm_mbar + tm.team);
+            }
+            tma_issued = true;
+        }
+    }
     // rows: all of them; columns: the live tiles of this step (Fin), spread evenly over the CTAs
     constexpr int CWL = CW == 8 ? 3 : (CW == 4 ? 2 : 0);
     typedef LiveCols<ROW ? 1 : (NX / kL)> LV;
@@ -456,7 +491,7 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
                 // load instruction, which kept the LSU busy for 0.5 us, become conflict-free LDS.
                 cf *stage = sm_y + tm.team * (TM::TEAM * 17);
                 unsigned long long *bar = sm_mbar + tm.team;
-                if (threadIdx.x % TM::TEAM == 0) {
+                if (threadIdx.x % TM::TEAM == 0 && !tma_issued) {
                     // the tile was written by other CTAs through the generic proxy (st.global) and the landing
                     // zone by this CTA: order both before the async-proxy copy
                     asm volatile("fence.proxy.async;" ::: "memory");
@@ -464,6 +499,7 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
 #pragma unroll
                     for (int cc = 0; cc < P; ++cc) tma_load_4d(stage + cc * kL * CW, &K.tmap, u * CW, cc, 0, b, bar);
                 }
+                tma_issued = false;                         // (only the first tile of a phase is requested early)
                 if (!mbar_wait(bar, uc.tma_parity)) {       // the copy never arrived: flag it and leave the phase; the grid
                     atomicExch(K.status, 2);                // barrier's watchdog sees the flag and ends the kernel
                     return;
