@@ -75,6 +75,8 @@ struct Plan {
     bool k8 = false;               // 8-point-thread kernel available for this shape
     bool k32 = false;              // 32-point-thread kernel (all shapes up to 1024; transform programs)
     bool force_k8 = false;         // BB_USE_K8=1 when the plan was made
+    // pupil of the last bb_multiplex_* call on this grid (pixel count and bounding box: an O(Nx Ny) host loop)
+    struct Pupil { float dx = 0.f, lambda = 0.f, na_in = -1.f, na = -1.f; long long count = 0; int Fx = 0, Wx = 0, Fy = 0, Wy = 0; } pupil;
     unsigned *bar = nullptr;
     int *status = nullptr;
     std::vector<TableEntry> tables;
@@ -1029,25 +1031,31 @@ int bb_multiplex_annular(const float *pos, const float *phase, const float *amp,
     // pupil pixel count, in double, same expression as the kernel's inside test
     const double ddx = dx, k0 = kTwoPi / (double)lambda, kc2 = (k0 * (double)NA) * (k0 * (double)NA);
     const double ki2 = (k0 * (double)NA_in) * (k0 * (double)NA_in);
-    long long count = 0;
-    std::vector<double> kx2(Nx), ky2(Ny);
-    for (int i = 0; i < Nx; ++i) { int f = (i < Nx / 2) ? i : i - Nx; double k = kTwoPi * (double)f / ((double)Nx * ddx); kx2[i] = k * k; }
-    for (int i = 0; i < Ny; ++i) { int f = (i < Ny / 2) ? i : i - Ny; double k = kTwoPi * (double)f / ((double)Ny * ddx); ky2[i] = k * k; }
-    for (int q = 0; q < Ny; ++q)
-        for (int i = 0; i < Nx; ++i)
-            if (kx2[i] + ky2[q] <= kc2 && kx2[i] + ky2[q] >= ki2) ++count;
+    if (!(p->pupil.dx == dx && p->pupil.lambda == lambda && p->pupil.na_in == NA_in && p->pupil.na == NA)) {
+        long long count = 0;
+        std::vector<double> kx2(Nx), ky2(Ny);
+        for (int i = 0; i < Nx; ++i) { int f = (i < Nx / 2) ? i : i - Nx; double k = kTwoPi * (double)f / ((double)Nx * ddx); kx2[i] = k * k; }
+        for (int i = 0; i < Ny; ++i) { int f = (i < Ny / 2) ? i : i - Ny; double k = kTwoPi * (double)f / ((double)Ny * ddx); ky2[i] = k * k; }
+        for (int q = 0; q < Ny; ++q)
+            for (int i = 0; i < Nx; ++i)
+                if (kx2[i] + ky2[q] <= kc2 && kx2[i] + ky2[q] >= ki2) ++count;
+        // bounding box of the pupil in DFT bins: [-F, F] per axis, clipped to [-N/2, N/2 - 1]
+        auto extent = [&](const std::vector<double> &k2, int N, int *lo, int *w) {
+            int F = 0;
+            for (int f = 0; f <= N / 2; ++f)
+                if (k2[f] <= kc2) F = f;
+            *lo = std::min(F, N / 2);
+            *w = *lo + std::min(F, N / 2 - 1) + 1;
+        };
+        Plan::Pupil pu;
+        pu.dx = dx; pu.lambda = lambda; pu.na_in = NA_in; pu.na = NA; pu.count = count;
+        extent(kx2, Nx, &pu.Fx, &pu.Wx);
+        extent(ky2, Ny, &pu.Fy, &pu.Wy);
+        p->pupil = pu;
+    }
+    const long long count = p->pupil.count;
     if (count == 0) return fail(BB_ERR_INVALID_ARG, "pupil of NA = %g contains no grid frequency", (double)NA);
-    // bounding box of the pupil in DFT bins: [-F, F] per axis, clipped to [-N/2, N/2 - 1]
-    auto extent = [&](const std::vector<double> &k2, int N, int *lo, int *w) {
-        int F = 0;
-        for (int f = 0; f <= N / 2; ++f)
-            if (k2[f] <= kc2) F = f;
-        *lo = std::min(F, N / 2);
-        *w = *lo + std::min(F, N / 2 - 1) + 1;
-    };
-    int Fx, Wx, Fy, Wy;
-    extent(kx2, Nx, &Fx, &Wx);
-    extent(ky2, Ny, &Fy, &Wy);
+    const int Fx = p->pupil.Fx, Wx = p->pupil.Wx, Fy = p->pupil.Fy, Wy = p->pupil.Wy;
     const size_t em_bytes = (((size_t)M * sizeof(bb::EmitterPrep)) + 255) & ~(size_t)255;
     DeviceCtx &ctx = device_ctx();
     rc = ws_reserve(ctx.misc, em_bytes + (size_t)M * (Wx + Wy) * sizeof(cf) + 4096);
