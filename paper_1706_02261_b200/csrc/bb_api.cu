@@ -75,6 +75,9 @@ struct Plan {
     bool k8 = false;               // 8-point-thread kernel available for this shape
     bool k32 = false;              // 32-point-thread kernel (all shapes up to 1024; transform programs)
     bool force_k8 = false;         // BB_USE_K8=1 when the plan was made
+    // diagnostic switches, read once when the plan is made (bb_shutdown + a new call re-reads them)
+    bool env_notma = false, env_noprune = false;
+    int env_cw = 0;                // BB_K16_CW: 4 or 8, 0 = automatic
     // pupil of the last bb_multiplex_* call on this grid (pixel count and bounding box: an O(Nx Ny) host loop)
     struct Pupil { float dx = 0.f, lambda = 0.f, na_in = -1.f, na = -1.f; long long count = 0; int Fx = 0, Wx = 0, Fy = 0, Wy = 0; } pupil;
     unsigned *bar = nullptr;
@@ -220,6 +223,9 @@ int get_plan(int Nx, int Ny, Plan **out) {
     }
     if (!p->k32 && !p->k8) { return fail(BB_ERR_UNSUPPORTED_SHAPE, "no kernel for Nx = %d, Ny = %d", Nx, Ny); }
     p->grid = sms;
+    p->env_notma = getenv("BB_K16_NOTMA") != nullptr;
+    p->env_noprune = getenv("BB_K16_NOPRUNE") != nullptr;
+    p->env_cw = getenv("BB_K16_CW") ? atoi(getenv("BB_K16_CW")) : 0;
     if (getenv("BB_GRID")) p->grid = std::max(1, std::min(sms, atoi(getenv("BB_GRID"))));   // diagnostic: persistent grid size
     guard.p = nullptr;
     g_plans.push_back(p);
@@ -286,7 +292,7 @@ void choose_tile_width(Plan *p, int B, int Nz, float dx, float lambda, float n0,
     double k0 = kTwoPi / (double)lambda;
     int F = 0;
     for (int j = 0; j < Nz; ++j) F = std::max(F, live_fmax(p->Nx, (double)dx, k0 * (double)(nref ? nref[j] : n0)));
-    if (getenv("BB_K16_CW")) { p->cw4 = atoi(getenv("BB_K16_CW")) == 4; return; }
+    if (p->env_cw) { p->cw4 = p->env_cw == 4; return; }
     p->cw4 = live_tiles(p->Nx, F, 4) * B <= p->grid;
 }
 
@@ -382,7 +388,7 @@ EncodeTiledFn encode_tiled_fn() {
 // fields [B][Ny][Nx] of 8-byte elements as (column, y mod PY, y div PY, field); box = (cw, 1, 256, 1)
 bool make_field_tmap(CUtensorMap *tm, void *field, int Nx, int Ny, int B, int cw) {
     EncodeTiledFn fn = encode_tiled_fn();
-    if (!fn || getenv("BB_K16_NOTMA")) return false;
+    if (!fn) return false;
     const int PY = Ny / 256;
     cuuint64_t dims[4] = {(cuuint64_t)Nx, (cuuint64_t)PY, 256, (cuuint64_t)B};
     cuuint64_t strides[3] = {(cuuint64_t)Nx * 8, (cuuint64_t)PY * Nx * 8, (cuuint64_t)Nx * Ny * 8};
@@ -435,7 +441,7 @@ int launch_steps(Plan *p, cf *field, const float *dn, float *inten, long long in
     P.noscreen = (flags & BB_HOMOGENEOUS) ? 1 : 0;
     const bool k8 = use_k8(p, B), k16 = use_k16(p, B);
     if (!k8 && !k16 && !p->k32) return fail(BB_ERR_UNSUPPORTED_SHAPE, "no kernel for Nx = %d, Ny = %d, batch = %d", p->Nx, p->Ny, B);
-    if (k16 || k8) P.use_tma = make_field_tmap(&P.tmap, field, p->Nx, p->Ny, B, p->cw4 ? 4 : 8) ? 1 : 0;
+    if (k16 || k8) P.use_tma = !p->env_notma && make_field_tmap(&P.tmap, field, p->Nx, p->Ny, B, p->cw4 ? 4 : 8) ? 1 : 0;
     if (g_trace && g_trace_dev == p->device && (k16 || k8) && 2 * Nz_total + 1 <= g_trace_phases) { P.trace = g_trace; P.trace_p0 = 0; }
     snprintf(g_last_kernel, sizeof g_last_kernel, k8 ? "bb::bpm8_kernel<%d,%d,%d,%s>" : k16 ? "bb::bpm16_kernel<%d,%d,%d,%s>" : "bb::bpm_kernel<%d,%d,%d>",
              k8 || k16 ? p->Nx / 256 : p->Nx / 32, k8 || k16 ? p->Ny / 256 : p->Ny / 32, k8 || k16 ? (p->cw4 ? 4 : 8) : 8,
@@ -479,7 +485,7 @@ int prepare_steps(Plan *p, int B, int Nz, int i0, float dx, float dz, float lamb
     unsigned long long protect = ++p->tick;
     const cf *last_ptr = nullptr;
     float last_nref = 0.f;
-    const bool noprune = getenv("BB_K16_NOPRUNE") != nullptr;
+    const bool noprune = p->env_noprune;
     int i = i0;
     for (; i < Nz; ++i) {
         const int j = backward ? Nz - 1 - i : i;
@@ -532,7 +538,7 @@ int run_program(Plan *p, cf *field, int B, const bb::PhaseProg *prog, int nprog,
         P.tw256 = p->tw256; P.twcx = p->twcx; P.twcy = p->twcy;
         P.xnat = 1;
         P.cw4 = p->Ny > 1024 ? 1 : 0;
-        P.use_tma = make_field_tmap(&P.tmap, field, p->Nx, p->Ny, B, P.cw4 ? 4 : 8) ? 1 : 0;
+        P.use_tma = !p->env_notma && make_field_tmap(&P.tmap, field, p->Nx, p->Ny, B, P.cw4 ? 4 : 8) ? 1 : 0;
         e = bb::kernel8_launch(p->Nx, p->Ny, P, p->grid, true, s);
     }
     ++g_launches;
