@@ -177,7 +177,13 @@ def time_propagation(bb, w, dev, field0_fn, dn, nref, inten, flags=0, runs=10, w
 def time_config(bb, dev, name, peaks, scratch, per_field=False, runs=10):
     """One entry of the `configs` array: a parity-test configuration timed the way SURVEY 8d asks
     (3 warm-ups, median and min of >= 10 runs, L2 flushed in between, plan and tables resident)."""
-    w = wl.config(name)
+    if name == "P31":
+        # the lateral grid of the paper's own runs (PAPER.md line 31: 1024 x 2048 x 1024 voxels), a slab of 128 slices:
+        # C4's recipe on 2048 x 1024 pixels -- 2048-point lines, the 8-point-thread kernel
+        import dataclasses
+        w = dataclasses.replace(wl.config("C4"), name="P31", Nx=2048, Nz=128, n_cells=500)
+    else:
+        w = wl.config(name)
     dn, f0, em = make_inputs(w, dev)
     nref = bb.nref_from_dn(dn, w.n0, w.nref_slab).numpy()
     if em is not None:
@@ -200,7 +206,7 @@ def time_config(bb, dev, name, peaks, scratch, per_field=False, runs=10):
     units = float(w.Nx) * w.Ny * w.Nz * B
     out = {"workload": "%s%s: %d field(s) of %dx%d, %d z-slices%s" % (w.name, " per-field intensity" if per_field else "", B, w.Nx, w.Ny, w.Nz,
                                                                      ", %.1f GiB intensity out" % (inten.numel() * 4 / 2**30) if per_field else ""),
-           "baseline_config": "BASELINE.json configs[%d]" % w.index,
+           "baseline_config": ("BASELINE.json configs[%d]" % w.index) if name != "P31" else "none: PAPER.md line 31 grid, C4 recipe",
            "propagate_ms": med, "propagate_ms_min": mn, "runs": len(ts),
            "value": units / (med * 1e-3) / 1e6, "unit": "Mvox/s", "kernel": bb.last_kernel(),
            "roofline": roofline_fracs(w, med * 1e-3, peaks, per_field)}
@@ -398,7 +404,7 @@ def run_ours(args):
         torch.cuda.empty_cache()
         scratch = torch.zeros(64 << 20, dtype=torch.float32, device=dev)          # 256 MiB
         cfgs = []
-        for name, per_field in (("C1", False), ("C2", False), ("C3", False), ("C5", False), ("C5", True)):
+        for name, per_field in (("C1", False), ("C2", False), ("C3", False), ("C5", False), ("C5", True), ("P31", False)):
             try:
                 cfgs.append(time_config(bb, dev, name, peaks, scratch, per_field=per_field))
             except Exception as e:                                        # noqa: BLE001
