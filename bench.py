@@ -179,7 +179,7 @@ def time_config(bb, dev, name, peaks, scratch, per_field=False, runs=10):
     (3 warm-ups, median and min of >= 10 runs, L2 flushed in between, plan and tables resident)."""
     if name == "P31":
         # the lateral grid of the paper's own runs (PAPER.md line 31: 1024 x 2048 x 1024 voxels), a slab of 128 slices:
-        # C4's recipe on 2048 x 1024 pixels -- 2048-point lines, the 8-point-thread kernel
+        # C4's recipe on 2048 x 1024 pixels -- 2048-point lines (class radix 8)
         import dataclasses
         w = dataclasses.replace(wl.config("C4"), name="P31", Nx=2048, Nz=128, n_cells=500)
     else:

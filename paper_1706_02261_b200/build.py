@@ -18,7 +18,7 @@ OBJ = os.path.join(HERE, "_build")
 LIB = os.path.join(HERE, "libbiobeam_b200.so")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 TXS = (1, 2, 4, 8, 16, 32)
-PXS = (1, 2, 4)
+PXS = (1, 2, 4, 8)
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I", INCLUDE]

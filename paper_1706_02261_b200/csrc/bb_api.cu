@@ -411,11 +411,11 @@ bool make_field_tmap(CUtensorMap *tm, void *field, int Nx, int Ny, int B, int cw
 
 // The 16-point-thread kernel serves single fields on 256/512/1024 grids; everything else (batches,
 // other shapes, the generic transform programs) runs on the 32-point-thread kernel.
-// 2048-point lines exist only in the 8-point-thread kernel; elsewhere the 16-point-thread kernel is
-// faster (profiles/r02_b) and the 8-point one is a diagnostic alternative (BB_USE_K8=1).
+// The 16-point-thread kernel is faster wherever both apply (profiles/r02_k8_kernel.md); the 8-point-thread one serves the
+// transform programs of 2048-point lines (run_program) and is a diagnostic alternative for propagations (BB_USE_K8=1).
 bool use_k8(const Plan *p, int B) {
     if (!p->k8) return false;
-    if (p->Nx <= 1024 && p->Ny <= 1024 && p->k16 && !p->force_k8) return false;
+    if (p->k16 && !p->force_k8) return false;
     const int rows = (p->Ny + p->grid - 1) / p->grid;
     return B == 1 || (long long)rows * p->Nx <= 8192;
 }
@@ -586,9 +586,10 @@ cudaError_t kernel_launch(int Nx, int Ny, const KParams &P, int grid, bool coop,
         case 1: return inst16_1_cw##cw##_b##bt##_##fn(__VA_ARGS__);   \
         case 2: return inst16_2_cw##cw##_b##bt##_##fn(__VA_ARGS__);   \
         case 4: return inst16_4_cw##cw##_b##bt##_##fn(__VA_ARGS__);   \
+        case 8: return inst16_8_cw##cw##_b##bt##_##fn(__VA_ARGS__);   \
     }
 bool kernel16_supports(int Nx, int Ny) {
-    auto ok = [](int n) { return n == 256 || n == 512 || n == 1024; };
+    auto ok = [](int n) { return n == 256 || n == 512 || n == 1024 || n == 2048; };
     return ok(Nx) && ok(Ny);
 }
 int kernel16_prepare(int Nx, int Ny) {

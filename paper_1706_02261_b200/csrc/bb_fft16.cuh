@@ -52,7 +52,7 @@ __device__ __forceinline__ void subline_fft(cf (&v)[16], const cf *__restrict__ 
     Dft<16, SIGN>::run(v);
 }
 
-// Radix-P butterfly over 4 consecutive registers of the 16 (P = 1, 2, 4), natural order in and out.
+// Radix-P butterfly over P consecutive registers of the 16 (P = 1, 2, 4, 8), natural order in and out.
 template <int P, int SIGN>
 __device__ __forceinline__ void class_dft(cf *w) {
     if constexpr (P == 2) {
@@ -67,6 +67,13 @@ __device__ __forceinline__ void class_dft(cf *w) {
         w[1] = cadd(b, d);
         w[2] = csub(a, c);
         w[3] = csub(b, d);
+    } else if constexpr (P == 8) {
+        cf v[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) v[i] = w[i];
+        Dft<8, SIGN>::run(v);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) w[i] = v[i];
     }
 }
 

@@ -10,29 +10,41 @@
 namespace bb {
 namespace {
 
+// a tile of 8 columns of a 2048-row grid would need a team of 1024 threads: such grids use tiles of 4
+template <int PY> constexpr bool valid16() { return 16 * PY * BB_CW <= kThreads16; }
+
 template <int PY>
 cudaError_t prepare_t() {
-    return cudaFuncSetAttribute(bpm16_kernel<BB_PX, PY, BB_CW, BB_BATCH != 0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)Smem16<BB_PX, PY>::bytes);
+    if constexpr (valid16<PY>())
+        return cudaFuncSetAttribute(bpm16_kernel<BB_PX, PY, BB_CW, BB_BATCH != 0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)Smem16<BB_PX, PY>::bytes);
+    else
+        return cudaSuccess;
 }
 template <int PY>
 int blocks_t() {
-    int n = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, bpm16_kernel<BB_PX, PY, BB_CW, BB_BATCH != 0>, kThreads16,
-                                                      Smem16<BB_PX, PY>::bytes) != cudaSuccess)
-        return 0;
+    int n = 1;
+    if constexpr (valid16<PY>()) {
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, bpm16_kernel<BB_PX, PY, BB_CW, BB_BATCH != 0>, kThreads16,
+                                                          Smem16<BB_PX, PY>::bytes) != cudaSuccess)
+            return 0;
+    }
     return n;
 }
 template <int PY>
 cudaError_t launch_t(const KParams &P, int grid, bool coop, cudaStream_t s) {
-    constexpr size_t smem = Smem16<BB_PX, PY>::bytes;
-    if (coop) {
-        void *args[] = {(void *)&P};
-        return cudaLaunchCooperativeKernel((const void *)bpm16_kernel<BB_PX, PY, BB_CW, BB_BATCH != 0>, dim3(grid), dim3(kThreads16),
-                                           args, smem, s);
+    if constexpr (valid16<PY>()) {
+        constexpr size_t smem = Smem16<BB_PX, PY>::bytes;
+        if (coop) {
+            void *args[] = {(void *)&P};
+            return cudaLaunchCooperativeKernel((const void *)bpm16_kernel<BB_PX, PY, BB_CW, BB_BATCH != 0>, dim3(grid), dim3(kThreads16),
+                                               args, smem, s);
+        }
+        bpm16_kernel<BB_PX, PY, BB_CW, BB_BATCH != 0><<<grid, kThreads16, smem, s>>>(P);
+        return cudaGetLastError();
+    } else {
+        return cudaErrorInvalidValue;
     }
-    bpm16_kernel<BB_PX, PY, BB_CW, BB_BATCH != 0><<<grid, kThreads16, smem, s>>>(P);
-    return cudaGetLastError();
 }
 
 }  // namespace
@@ -44,6 +56,7 @@ cudaError_t launch_t(const KParams &P, int grid, bool coop, cudaStream_t s) {
         case 1: return expr_prefix<1>(__VA_ARGS__);  \
         case 2: return expr_prefix<2>(__VA_ARGS__);  \
         case 4: return expr_prefix<4>(__VA_ARGS__);  \
+        case 8: return expr_prefix<8>(__VA_ARGS__);  \
     }
 
 cudaError_t BB_CAT(inst16_, BB_PX, _cw, BB_CW, _b, BB_BATCH, _prepare)(int PY) {

@@ -1,4 +1,4 @@
-// bb_kernels16.cuh -- the BPM step kernel with 16 points per thread (Nx, Ny in {256, 512, 1024}; single fields and batches).
+// bb_kernels16.cuh -- the BPM step kernel with 16 points per thread (Nx, Ny in {256, 512, 1024, 2048}; single fields and batches).
 //
 // Same two-phase structure as bb_kernels.cuh:
 //   column phase C_j : FFT_y  -> x H_j                          -> IFFT_y

@@ -18,16 +18,16 @@ BB_DECLARE_INST(16)
 BB_DECLARE_INST(32)
 #undef BB_DECLARE_INST
 
-// 16-point-thread kernel (bb_kernels16.cuh), one set per PX = Nx/256 in {1, 2, 4} and column
+// 16-point-thread kernel (bb_kernels16.cuh), one set per PX = Nx/256 in {1, 2, 4, 8} and column
 // tile width in {4, 8}; bb_inst16.cu.
 #define BB_DECLARE_INST16(PX, CW, BT)                                                                              \
     cudaError_t inst16_##PX##_cw##CW##_b##BT##_prepare(int PY);                                                     \
     int inst16_##PX##_cw##CW##_b##BT##_blocks_per_sm(int PY);                                                       \
     cudaError_t inst16_##PX##_cw##CW##_b##BT##_launch(int PY, const KParams &P, int grid, bool coop, cudaStream_t s);
-BB_DECLARE_INST16(1, 4, 0) BB_DECLARE_INST16(2, 4, 0) BB_DECLARE_INST16(4, 4, 0)
-BB_DECLARE_INST16(1, 8, 0) BB_DECLARE_INST16(2, 8, 0) BB_DECLARE_INST16(4, 8, 0)
-BB_DECLARE_INST16(1, 4, 1) BB_DECLARE_INST16(2, 4, 1) BB_DECLARE_INST16(4, 4, 1)
-BB_DECLARE_INST16(1, 8, 1) BB_DECLARE_INST16(2, 8, 1) BB_DECLARE_INST16(4, 8, 1)
+BB_DECLARE_INST16(1, 4, 0) BB_DECLARE_INST16(2, 4, 0) BB_DECLARE_INST16(4, 4, 0) BB_DECLARE_INST16(8, 4, 0)
+BB_DECLARE_INST16(1, 8, 0) BB_DECLARE_INST16(2, 8, 0) BB_DECLARE_INST16(4, 8, 0) BB_DECLARE_INST16(8, 8, 0)
+BB_DECLARE_INST16(1, 4, 1) BB_DECLARE_INST16(2, 4, 1) BB_DECLARE_INST16(4, 4, 1) BB_DECLARE_INST16(8, 4, 1)
+BB_DECLARE_INST16(1, 8, 1) BB_DECLARE_INST16(2, 8, 1) BB_DECLARE_INST16(4, 8, 1) BB_DECLARE_INST16(8, 8, 1)
 #undef BB_DECLARE_INST16
 
 // 8-point-thread kernel (bb_kernels8.cuh), one set per PX = Nx/256 in {1, 2, 4, 8} and column tile width in

@@ -24,7 +24,7 @@ def _case(Nx, Ny, Nz, B, seed=3):
     return w, dn, f0
 
 
-# ---------------------------------------------------------------- 2048-point lines (8-point-thread kernel)
+# ---------------------------------------------------------------- 2048-point lines (class radix 8)
 @pytest.mark.parametrize("Nx,Ny,Nz,B", [(2048, 256, 2, 1), (256, 2048, 2, 1), (2048, 1024, 2, 1), (1024, 2048, 2, 1),
                                          (2048, 2048, 2, 1), (2048, 512, 3, 2)])
 def test_2048_point_lines(oracle_mod, Nx, Ny, Nz, B):
@@ -44,14 +44,19 @@ def test_2048_point_lines(oracle_mod, Nx, Ny, Nz, B):
     assert rel_l2(I.cpu().numpy(), Io) < 2 * small_tol(Nz)
 
 
-@pytest.mark.parametrize("cfg", ["C2", "C3"])
-def test_8_point_thread_kernel_on_smaller_grids(oracle_mod, monkeypatch, cfg):
-    """BB_USE_K8=1 routes 256 / 512 / 1024 grids to the kernel that 2048-point lines use."""
+@pytest.mark.parametrize("cfg", ["C2", "C3", "2048x512", "512x2048"])
+def test_8_point_thread_kernel(oracle_mod, monkeypatch, cfg):
+    """BB_USE_K8=1 routes propagations to the 8-point-thread kernel (otherwise it only runs the transform
+    programs of 2048-point lines): every class radix, 1 .. 8."""
     bb = need_gpu()
     bb.shutdown()
     monkeypatch.setenv("BB_USE_K8", "1")
     try:
-        w = wl.config(cfg).with_nz(6)
+        if "x" in cfg:
+            nx, ny = (int(v) for v in cfg.split("x"))
+            w = wl.dataclasses.replace(wl.tiny(N=nx, Nz=6, n_cells=10, r_lo=0.5, r_hi=3.0), Ny=ny, nref_slab=2)
+        else:
+            w = wl.config(cfg).with_nz(6)
         dn = wl.make_dn(w)
         f0 = wl.random_field(w.Nx, w.Ny, seed=5, batch=1)
         nref = oracle_mod.nref_from_dn(dn.numpy(), w.n0, 2)
@@ -59,6 +64,7 @@ def test_8_point_thread_kernel_on_smaller_grids(oracle_mod, monkeypatch, cfg):
         I = torch.empty((6, w.Ny, w.Nx), device="cuda")
         bb.propagate(d, dn.cuda(), w.dx, w.dz, w.lam, w.n0, intensity=I, nref=nref)
         torch.cuda.synchronize()
+        assert "bpm8_kernel" in bb.last_kernel()
         uo, Io = oracle_mod.propagate(f0[0], dn.numpy(), w.dx, w.dz, w.lam, w.n0, nref=nref)
         assert rel_l2(d[0].cpu().numpy(), uo) < small_tol(6)
         assert rel_l2(I.cpu().numpy(), Io) < 2 * small_tol(6)
