@@ -99,9 +99,9 @@ int bb_propagate(void *field, const float *dn_volume, int Nx, int Ny, int Nz,
 /* Same with options (batch, adapted n_ref, accumulate / per-field intensity, backward, homogeneous,
  * stream).  opts may be NULL.  Kernel selection (results do not depend on it beyond rounding): grids
  * with sides in {256, 512, 1024, 2048} run the 16-point-thread kernel -- for a batch only while the screen
- * factors of a CTA's rows fit its buffer, ceil(Ny / SMs) * Nx <= 8192 (a batch on a grid with a 2048-point
- * side that exceeds it is BB_ERR_UNSUPPORTED_SHAPE) -- everything else the 32-point-thread kernel (sides up to
- * 1024).  The 8-point-thread kernel runs the transforms of bb_fft2 / bb_multiplex_* on grids with a 2048-point
+ * factors of a CTA's rows fit its buffer, ceil(Ny / SMs) * Nx <= 8192; a larger batch runs field by field
+ * on the single-field variant (dn is then read once per field) -- everything else the 32-point-thread kernel
+ * (sides up to 1024).  The 8-point-thread kernel runs the transforms of bb_fft2 / bb_multiplex_* on grids with a 2048-point
  * side and, with BB_USE_K8=1 in the environment, propagations.  The summed intensity of a
  * batch is accumulated with shared-memory atomics: its summation order, hence its last bits, can
  * differ between runs (tolerance contract: relative L2 <= 1e-4 against the definition). */

@@ -718,6 +718,23 @@ int propagate_impl(void *field, const float *dn, int Nx, int Ny, int Nz, float d
     if (rc) return rc;
     cudaStream_t s = opts ? (cudaStream_t)opts->stream : (cudaStream_t)0;
     const float *nref = opts ? opts->nref : nullptr;
+    // A batch the batch variant of the 16-point-thread kernel cannot take (the screen factors of a CTA's rows
+    // must fit one buffer) runs field by field on its single-field variant -- faster than the 32-point-thread
+    // kernel, and the only way on a grid with a 2048-point side; dn is then read once per field.
+    if (B > 1 && p->k16 && !use_k16(p, B) && !use_k8(p, B)) {
+        const size_t npx1 = (size_t)Nx * Ny;
+        for (int b = 0; b < B; ++b) {
+            bb_opts o = *opts;
+            o.batch = 1;
+            o.flags = flags & ~BB_INTENSITY_PER_FIELD;
+            float *I = intensity_out;
+            if (intensity_out && (flags & BB_INTENSITY_PER_FIELD)) I = intensity_out + (size_t)b * Nz * npx1;
+            else if (b > 0) o.flags |= BB_ACCUMULATE;          // summed over the batch
+            rc = propagate_impl((cf *)field + (size_t)b * npx1, dn, Nx, Ny, Nz, dx, dz, lambda, n0, I, &o, allow_zero_dz);
+            if (rc) return rc;
+        }
+        return BB_OK;
+    }
     choose_tile_width(p, B, Nz, dx, lambda, n0, nref);
     std::vector<const cf *> h_tab(Nz);
     std::vector<float> h_phase(Nz);

@@ -44,6 +44,30 @@ def test_2048_point_lines(oracle_mod, Nx, Ny, Nz, B):
     assert rel_l2(I.cpu().numpy(), Io) < 2 * small_tol(Nz)
 
 
+@pytest.mark.parametrize("Nx,Ny,B,per_field", [(2048, 1024, 2, False), (1024, 2048, 3, True)])
+def test_batches_too_large_for_the_batch_kernel_run_field_by_field(oracle_mod, Nx, Ny, B, per_field):
+    """ceil(Ny / SMs) * Nx > 8192: the batch variant cannot hold the screen factors of a CTA's rows; summed and
+    per-field intensities, on top of existing contents (BB_ACCUMULATE)."""
+    bb = need_gpu()
+    Nz = 2
+    w, dn, f0 = _case(Nx, Ny, Nz, B, seed=17)
+    nref = oracle_mod.nref_from_dn(dn.numpy(), w.n0, 1)
+    d = torch.from_numpy(f0).cuda()
+    shape = ((B,) if per_field else ()) + (Nz, Ny, Nx)
+    I0 = np.random.default_rng(1).uniform(0, 1, size=shape).astype(np.float32)
+    I = torch.from_numpy(I0).cuda()
+    flags = bb.ACCUMULATE | (bb.INTENSITY_PER_FIELD if per_field else 0)
+    bb.propagate(d, dn.cuda(), w.dx, w.dz, w.lam, w.n0, intensity=I, nref=nref, flags=flags)
+    torch.cuda.synchronize()
+    assert "false" in bb.last_kernel()                      # the single-field variant did the work
+    Io = np.zeros((B, Nz, Ny, Nx))
+    for b in range(B):
+        uo, Io[b] = oracle_mod.propagate(f0[b], dn.numpy(), w.dx, w.dz, w.lam, w.n0, nref=nref)
+        assert rel_l2(d[b].cpu().numpy(), uo) < small_tol(Nz)
+    expect = (Io if per_field else Io.sum(axis=0)) + I0.astype(np.float64)
+    assert rel_l2(I.cpu().numpy(), expect) < 2 * small_tol(Nz)
+
+
 @pytest.mark.parametrize("cfg", ["C2", "C3", "2048x512", "512x2048"])
 def test_8_point_thread_kernel(oracle_mod, monkeypatch, cfg):
     """BB_USE_K8=1 routes propagations to the 8-point-thread kernel (otherwise it only runs the transform
