@@ -855,9 +855,21 @@ int bb_image_formation(const float *source, int Nx, int Ny, const float *emitter
     return BB_OK;
 }
 
+}  // extern "C"
+namespace {
+int propagate_host_impl(void *field_host, const float *dn_host, int Nx, int Ny, int Nz, float dx, float dz,
+                        float lambda, float n0, float *inten_host, const bb_opts *opts);
+}
+extern "C" {
 int bb_propagate_host(void *field_host, const float *dn_host, int Nx, int Ny, int Nz, float dx, float dz,
                       float lambda, float n0, float *inten_host, const bb_opts *opts) {
     std::lock_guard<std::mutex> lk(g_mu);
+    return propagate_host_impl(field_host, dn_host, Nx, Ny, Nz, dx, dz, lambda, n0, inten_host, opts);
+}
+}  // extern "C"
+namespace {
+int propagate_host_impl(void *field_host, const float *dn_host, int Nx, int Ny, int Nz, float dx, float dz,
+                        float lambda, float n0, float *inten_host, const bb_opts *opts) {
     int B; unsigned flags;
     int rc = validate_common(field_host, dn_host, Nx, Ny, Nz, dx, dz, lambda, n0, opts, &B, &flags);
     if (rc) return rc;
@@ -866,6 +878,20 @@ int bb_propagate_host(void *field_host, const float *dn_host, int Nx, int Ny, in
     if (rc) return rc;
     DeviceCtx &ctx = device_ctx();
     const float *nref = opts ? opts->nref : nullptr;
+    if (B > 1 && p->k16 && !use_k16(p, B) && !use_k8(p, B)) {       // as in propagate_impl: field by field
+        const size_t npx1 = (size_t)Nx * Ny;
+        for (int b = 0; b < B; ++b) {
+            bb_opts o = *opts;
+            o.batch = 1;
+            o.flags = flags & ~BB_INTENSITY_PER_FIELD;
+            float *I = inten_host;
+            if (inten_host && (flags & BB_INTENSITY_PER_FIELD)) I = inten_host + (size_t)b * Nz * npx1;
+            else if (b > 0) o.flags |= BB_ACCUMULATE;
+            rc = propagate_host_impl((cf *)field_host + (size_t)b * npx1, dn_host, Nx, Ny, Nz, dx, dz, lambda, n0, I, &o);
+            if (rc) return rc;
+        }
+        return BB_OK;
+    }
     choose_tile_width(p, B, Nz, dx, lambda, n0, nref);
     const size_t npx = (size_t)Nx * Ny;
     const bool per_field = (flags & BB_INTENSITY_PER_FIELD) != 0;
@@ -961,6 +987,9 @@ int bb_propagate_host(void *field_host, const float *dn_host, int Nx, int Ny, in
     }
     return result;
 }
+
+}  // namespace
+extern "C" {
 
 int bb_nref_from_dn(const float *dn, int Nx, int Ny, int Nz, float n0, int slab, float *nref_out, void *stream) {
     std::lock_guard<std::mutex> lk(g_mu);

@@ -66,6 +66,11 @@ def test_batches_too_large_for_the_batch_kernel_run_field_by_field(oracle_mod, N
         assert rel_l2(d[b].cpu().numpy(), uo) < small_tol(Nz)
     expect = (Io if per_field else Io.sum(axis=0)) + I0.astype(np.float64)
     assert rel_l2(I.cpu().numpy(), expect) < 2 * small_tol(Nz)
+    # the host-buffer entry point takes the same route: bit-identical
+    fh = torch.from_numpy(f0.copy()).pin_memory()
+    Ih = torch.from_numpy(I0.copy()).pin_memory()
+    bb.propagate(fh, dn.pin_memory(), w.dx, w.dz, w.lam, w.n0, intensity=Ih, nref=nref, flags=flags)
+    assert torch.equal(fh, d.cpu()) and torch.equal(Ih, I.cpu())
 
 
 @pytest.mark.parametrize("cfg", ["C2", "C3", "2048x512", "512x2048"])
