@@ -491,15 +491,18 @@ __device__ __forceinline__ void run_phase16(const KParams &K, const Phase16 &d, 
                 // load instruction, which kept the LSU busy for 0.5 us, become conflict-free LDS.
                 cf *stage = sm_y + tm.team * (TM::TEAM * 17);
                 unsigned long long *bar = sm_mbar + tm.team;
-                if (threadIdx.x % TM::TEAM == 0 && !tma_issued) {
-                    // the tile was written by other CTAs through the generic proxy (st.global) and the landing
-                    // zone by this CTA: order both before the async-proxy copy
-                    asm volatile("fence.proxy.async;" ::: "memory");
+                if (threadIdx.x % TM::TEAM == 0 && (BATCH || !tma_issued)) {
+                    // the tiles were written by other CTAs through the generic proxy (st.global, before the grid
+                    // barrier) and the landing zone by this CTA: order both before the async-proxy copy.  The
+                    // full proxy fence is needed once per phase (it costs ~0.1 us); later tiles only have to order
+                    // this CTA's own shared-memory accesses.
+                    if (k == k0 + tm.team) asm volatile("fence.proxy.async;" ::: "memory");
+                    else asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                     mbar_expect_tx(bar, (unsigned)(P * kL * CW * sizeof(cf)));
 #pragma unroll
                     for (int cc = 0; cc < P; ++cc) tma_load_4d(stage + cc * kL * CW, &K.tmap, u * CW, cc, 0, b, bar);
                 }
-                tma_issued = false;                         // (only the first tile of a phase is requested early)
+                if constexpr (!BATCH) tma_issued = false;   // (only the first tile of a phase is requested early)
                 if (!mbar_wait(bar, uc.tma_parity)) {       // the copy never arrived: flag it and leave the phase; the grid
                     atomicExch(K.status, 2);                // barrier's watchdog sees the flag and ends the kernel
                     return;

@@ -239,9 +239,10 @@ __device__ __forceinline__ void run_phase8(const KParams &K, const Phase16 &d, c
                 cf *stage = sm_y + tm.team * (TM::TEAM / 32) * (16 * 17);
                 unsigned long long *bar = sm_mbar + tm.team;
                 if (threadIdx.x % TM::TEAM == 0) {
-                    // the tile was written by other CTAs through the generic proxy (st.global) and the landing
-                    // zone by this CTA: order both before the async-proxy copy
-                    asm volatile("fence.proxy.async;" ::: "memory");
+                    // the tiles were written by other CTAs through the generic proxy (st.global) and the landing
+                    // zone by this CTA: order both before the async-proxy copy (full fence once per phase)
+                    if (k == k0 + tm.team) asm volatile("fence.proxy.async;" ::: "memory");
+                    else asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                     mbar_expect_tx(bar, (unsigned)(P * kL * CW * sizeof(cf)));
 #pragma unroll
                     for (int cc = 0; cc < P; ++cc) tma_load_4d(stage + cc * kL * CW, &K.tmap, u * CW, cc, 0, b, bar);
