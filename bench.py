@@ -214,6 +214,68 @@ def time_config(bb, dev, name, peaks, scratch, per_field=False, runs=10):
     return out
 
 
+def time_next_rows(bb, dev, peaks, runs=10):
+    """The NEXT rows of SURVEY 8f, each timed on a C3/C4-sized input (median of `runs` after 3 warm-ups, CUDA events)
+    with the roofline that bounds it: algorithmic bytes or flops over the measured duration."""
+    def timed(fn):
+        ts = []
+        for i in range(3 + runs):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); fn(); b.record()
+            torch.cuda.synchronize()
+            if i >= 3:
+                ts.append(a.elapsed_time(b))
+        return statistics.median(ts)
+
+    out = []
+    hbm = peaks["hbm"]
+    # NEXT-4 backward propagation: C4's grid and phantom recipe, 64 slices, n_ref slabs of 32
+    w = wl.config("C4").with_nz(64)
+    dn, _, em = make_inputs(w, dev)
+    nref = bb.nref_from_dn(dn, w.n0, w.nref_slab).numpy()
+    f = bb.multiplex_psf(*(t.to(dev) for t in em), w.NA, w.Nx, w.Ny, w.dx, w.lam)[None].contiguous()
+    I = torch.empty((w.Nz, w.Ny, w.Nx), device=dev)
+    for name, flags in (("forward, for comparison", 0), ("BB_BACKWARD", bb.BACKWARD)):
+        ms = timed(lambda: bb.propagate(f, dn, w.dx, w.dz, w.lam, w.n0, intensity=I, nref=nref, flags=flags))
+        out.append({"row": "NEXT-4", "what": "%s: 1024x1024, 64 slices" % name, "ms": ms, "kernel": bb.last_kernel(),
+                    "roofline": roofline_fracs(w, ms * 1e-3, peaks)})
+    # NEXT-1: refocus (one H-only step), through-focus stack (64 homogeneous steps with intensity), PSF tiles
+    ms = timed(lambda: bb.refocus(f, w.dx, -6.4, w.lam, w.n0))
+    out.append({"row": "NEXT-1", "what": "bb_refocus: 1024x1024, one signed step", "ms": ms,
+                "note": "three phases of the persistent kernel (two grid barriers): latency-bound, %.1f us" % (ms * 1e3)})
+    ms = timed(lambda: bb.propagate(f, None, w.dx, w.dz, w.lam, w.n0, intensity=I, flags=bb.HOMOGENEOUS, nz=w.Nz))
+    wh = w
+    out.append({"row": "NEXT-1", "what": "BB_HOMOGENEOUS through-focus stack: 1024x1024, 64 planes", "ms": ms,
+                "roofline": roofline_fracs(wh, ms * 1e-3, peaks)})
+    pos = em[0].to(dev)
+    T = 32
+    tiles = None
+    def do_tiles():
+        nonlocal tiles
+        tiles = bb.extract_tiles(I, pos, w.dx, T)
+    ms = timed(do_tiles)
+    nbytes = 2 * pos.shape[0] * w.Nz * T * T * 4
+    out.append({"row": "NEXT-1", "what": "bb_extract_tiles: %d emitters x 64 planes x 32x32 floats" % pos.shape[0], "ms": ms,
+                "roofline": {"bound": "hbm", "achieved_gbs": nbytes / (ms * 1e-3) / 1e9, "peak_gbs": hbm,
+                             "frac": nbytes / (ms * 1e-3) / 1e9 / hbm, "algorithmic_bytes": nbytes}})
+    # NEXT-2: generators
+    ms = timed(lambda: bb.lightsheet(1024, 1024, 0.1, 0.5, 1.33, 0.2, 25.6, device=dev))
+    out.append({"row": "NEXT-2", "what": "bb_lightsheet: 1024x1024 (fill + one back-propagation step)", "ms": ms,
+                "note": "latency-bound like bb_refocus"})
+    ms = timed(lambda: bb.multiplex_annular(pos, em[1].to(dev), None, 0.55, 0.6, w.Nx, w.Ny, w.dx, w.lam))
+    out.append({"row": "NEXT-2", "what": "bb_multiplex_annular: 1024 Bessel foci on 1024x1024, NA 0.55-0.6", "ms": ms})
+    # NEXT-3: image formation, 1024x1024 source, 32x32 emitter grid, 32x32 tiles: 2 T^2 flop per pixel
+    S = torch.rand((w.Ny, w.Nx), device=dev)
+    psf = torch.rand((pos.shape[0], T, T), device=dev)
+    ms = timed(lambda: bb.image_formation(S, pos, w.dx, psf))
+    flop = 2.0 * w.Nx * w.Ny * T * T
+    out.append({"row": "NEXT-3", "what": "bb_image_formation: 1024x1024, %d PSF tiles of 32x32" % pos.shape[0], "ms": ms,
+                "roofline": {"bound": "alu", "achieved_tflops": flop / (ms * 1e-3) / 1e12, "peak_tflops": FP32_PEAK_TFLOPS,
+                             "frac": flop / (ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS, "algorithmic_flop": flop,
+                             "note": "includes the nearest-emitter map (1024 distance tests per pixel in double)"}})
+    return out
+
+
 def run_ours(args):
     from paper_1706_02261_b200 import binding as bb, build
     rank, local_rank, _ = replicas.env_world()
@@ -410,6 +472,10 @@ def run_ours(args):
             except Exception as e:                                        # noqa: BLE001
                 cfgs.append({"workload": name, "error": str(e)})
         result["configs"] = cfgs
+        try:
+            result["next_rows"] = time_next_rows(bb, dev, peaks)
+        except Exception as e:                                            # noqa: BLE001
+            result["next_rows"] = [{"error": str(e)}]
         result["configs_note"] = ("3 warm-ups, median (propagate_ms) and min of 10 propagations each, 256 MiB written between runs; "
                                   "C1-C3 are latency-bound (T_roof is sub-microsecond per step): their fractions are for information")
 

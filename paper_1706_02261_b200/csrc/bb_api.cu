@@ -795,7 +795,7 @@ int bb_extract_tiles(const void *src, int elem, int Nx, int Ny, int Nplanes, con
     int dev, sms;
     int rc = check_arch(&dev, &sms);
     if (rc) return rc;
-    dim3 grid((T * T + 255) / 256, Nplanes, M);
+    dim3 grid(Nplanes, M);
     if (elem == 1)
         bb::extract_tiles_kernel<1><<<grid, 256, 0, (cudaStream_t)stream>>>((const float *)src, Nx, Ny, Nplanes, emitter_positions, M, (double)dx, T, (float *)tiles_out);
     else
@@ -833,23 +833,29 @@ int bb_image_formation(const float *source, int Nx, int Ny, const float *emitter
                        const float *psf_tiles, int T, float *image_out, void *stream) {
     std::lock_guard<std::mutex> lk(g_mu);
     if (!source || !emitter_positions || !psf_tiles || !image_out) return fail(BB_ERR_INVALID_ARG, "a pointer argument is NULL");
-    if (Nx < 1 || Ny < 1 || M < 1 || Ny > 65535) return fail(BB_ERR_INVALID_ARG, "Nx, Ny, M must be >= 1 (Ny <= 65535)");
+    if (Nx < 1 || Ny < 1 || M < 1 || M > 65535) return fail(BB_ERR_INVALID_ARG, "Nx, Ny, M must be >= 1 (M <= 65535)");
     if (T < 1 || T > Nx || T > Ny || T > 96) return fail(BB_ERR_INVALID_ARG, "tile size T = %d must be in [1, min(Nx, Ny, 96)]", T);
     if (!(dx > 0.f) || !std::isfinite(dx)) return fail(BB_ERR_INVALID_ARG, "dx must be positive and finite");
     int dev, sms;
     int rc = check_arch(&dev, &sms);
     if (rc) return rc;
     DeviceCtx &ctx = device_ctx();
-    rc = ws_reserve(ctx.misc, (size_t)Nx * Ny * sizeof(int));
+    const size_t own_bytes = (((size_t)Nx * Ny * sizeof(int)) + 255) & ~(size_t)255;
+    rc = ws_reserve(ctx.misc, own_bytes + (size_t)M * (Nx + Ny) * sizeof(double));
     if (rc) return rc;
     int *owner = (int *)ctx.misc.ptr;
+    double *dx2 = (double *)((char *)ctx.misc.ptr + own_bytes), *dy2 = dx2 + (size_t)M * Nx;
     cudaStream_t s = (cudaStream_t)stream;
-    bb::nearest_emitter_kernel<<<dim3((Nx + 127) / 128, Ny), 128, 0, s>>>(Nx, Ny, emitter_positions, M, (double)dx, owner);
-    ++g_launches;
-    const size_t smem = (size_t)(32 + T - 1) * (8 + T - 1) * 8;
+    bb::emitter_axis_dist2_kernel<<<dim3((Nx + 127) / 128, M), 128, 0, s>>>(Nx, emitter_positions, 0, M, (double)dx, dx2);
+    bb::emitter_axis_dist2_kernel<<<dim3((Ny + 127) / 128, M), 128, 0, s>>>(Ny, emitter_positions, 1, M, (double)dx, dy2);
+    bb::nearest_emitter_kernel<<<dim3((Nx + 127) / 128, (Ny + 7) / 8), 128, 0, s>>>(Nx, Ny, M, dx2, dy2, owner);
+    g_launches += 3;
+    const size_t halo = (size_t)(32 + T - 1) * (8 + T - 1) * 8, tile = (size_t)T * T * sizeof(float);
+    const int K = (int)std::max<size_t>(0, std::min<size_t>(16, ((size_t)160 * 1024 - halo) / tile));   // staged tiles per CTA
+    const size_t smem = halo + (size_t)K * tile;
     if (smem > 48 * 1024)
         BB_CUDA(cudaFuncSetAttribute(bb::image_formation_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    bb::image_formation_kernel<<<dim3((Nx + 31) / 32, (Ny + 7) / 8), 256, smem, s>>>(source, owner, Nx, Ny, psf_tiles, T, image_out);
+    bb::image_formation_kernel<<<dim3((Nx + 31) / 32, (Ny + 7) / 8), 256, smem, s>>>(source, owner, Nx, Ny, psf_tiles, T, K, image_out);
     ++g_launches;
     BB_CUDA(cudaGetLastError());
     return BB_OK;

@@ -147,19 +147,24 @@ __global__ void slice_sum_kernel(const float *__restrict__ dn, size_t npx, doubl
 
 // T x T windows around the emitters of every plane of a stack (bb_extract_tiles): out[e][z][ty][tx] =
 // src[z][(cy - T/2 + ty) mod Ny][(cx - T/2 + tx) mod Nx], (cx, cy) = nearest pixel of emitter e; ELEM floats per pixel.
+// One CTA per (emitter, plane): window origin once per CTA, 32-bit index arithmetic, rows of T contiguous pixels.
 template <int ELEM>
-__global__ void extract_tiles_kernel(const float *__restrict__ src, int Nx, int Ny, int Np, const float *__restrict__ pos,
-                                     int M, double dx, int T, float *__restrict__ out) {
-    const int e = blockIdx.z, z = blockIdx.y;
+__global__ void __launch_bounds__(256) extract_tiles_kernel(const float *__restrict__ src, int Nx, int Ny, int Np,
+                                                            const float *__restrict__ pos, int M, double dx, int T,
+                                                            float *__restrict__ out) {
+    const int e = blockIdx.y, z = blockIdx.x;
     const long long cx = (long long)floor(__ddiv_rn((double)pos[2 * e], dx) + 0.5) + Nx / 2;
     const long long cy = (long long)floor(__ddiv_rn((double)pos[2 * e + 1], dx) + 0.5) + Ny / 2;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < T * T; i += gridDim.x * blockDim.x) {
-        const int ty = i / T, tx = i - ty * T;
-        const long long x = ((cx - T / 2 + tx) % Nx + Nx) % Nx, y = ((cy - T / 2 + ty) % Ny + Ny) % Ny;
-        const float *sp = src + (((size_t)z * Ny + y) * Nx + x) * ELEM;
-        float *op = out + ((((size_t)e * Np + z) * T + ty) * T + tx) * ELEM;
-#pragma unroll
-        for (int c = 0; c < ELEM; ++c) op[c] = sp[c];
+    const int x0 = (int)(((cx - T / 2) % Nx + Nx) % Nx), y0 = (int)(((cy - T / 2) % Ny + Ny) % Ny);
+    const float *plane = src + (size_t)z * Ny * Nx * ELEM;
+    float *op = out + ((size_t)e * Np + z) * T * T * ELEM;
+    const int n = T * T * ELEM, rowlen = T * ELEM;
+    for (int i = threadIdx.x; i < n; i += 256) {
+        const int ty = i / rowlen, r = i - ty * rowlen, tx = r / ELEM, c = r - tx * ELEM;
+        int x = x0 + tx, y = y0 + ty;
+        if (x >= Nx) x -= Nx;
+        if (y >= Ny) y -= Ny;
+        op[i] = plane[((size_t)y * Nx + x) * ELEM + c];
     }
 }
 
@@ -172,35 +177,80 @@ __global__ void gaussian_sheet_kernel(float2 *__restrict__ u, int Nx, int Ny, do
 }
 
 // Image formation (bb_image_formation), step 1: the emitter nearest to every pixel (periodic distance, lowest
-// index on ties; double, no fused multiply-adds: the comparison is a decision).
-__global__ void nearest_emitter_kernel(int Nx, int Ny, const float *__restrict__ pos, int M, double dx, int *__restrict__ owner) {
-    const int x = blockIdx.x * blockDim.x + threadIdx.x, y = blockIdx.y;
-    if (x >= Nx) return;
-    const double px = __dmul_rn((double)(x - Nx / 2), dx), py = __dmul_rn((double)(y - Ny / 2), dx);
-    const double Lx = __dmul_rn((double)Nx, dx), Ly = __dmul_rn((double)Ny, dx);
-    int best = 0;
-    double bd = 0.0;
-    for (int e = 0; e < M; ++e) {
-        double ddx = __dsub_rn(px, (double)pos[2 * e]), ddy = __dsub_rn(py, (double)pos[2 * e + 1]);
-        ddx = __dsub_rn(ddx, __dmul_rn(Lx, floor(__dadd_rn(__ddiv_rn(ddx, Lx), 0.5))));
-        ddy = __dsub_rn(ddy, __dmul_rn(Ly, floor(__dadd_rn(__ddiv_rn(ddy, Ly), 0.5))));
-        const double d2 = __dadd_rn(__dmul_rn(ddx, ddx), __dmul_rn(ddy, ddy));
-        if (e == 0 || d2 < bd) { bd = d2; best = e; }
+// index on ties; double, no fused multiply-adds: the comparison is a decision).  The squared distance separates,
+// d2 = ddx^2 + ddy^2 with ddx a function of (x, emitter) and ddy of (y, emitter): the expensive part (a division and
+// a floor per component) is tabulated per axis, the per-pixel search is one addition and one comparison per emitter.
+//   axis2[e][i] = (d - L floor(d / L + 0.5))^2,  d = (i - N/2) dx - pos[e][axis]
+__global__ void emitter_axis_dist2_kernel(int N, const float *__restrict__ pos, int axis, int M, double dx, double *__restrict__ out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, e = blockIdx.y;
+    if (i >= N) return;
+    const double L = __dmul_rn((double)N, dx);
+    double d = __dsub_rn(__dmul_rn((double)(i - N / 2), dx), (double)pos[2 * e + axis]);
+    d = __dsub_rn(d, __dmul_rn(L, floor(__dadd_rn(__ddiv_rn(d, L), 0.5))));
+    out[(size_t)e * N + i] = __dmul_rn(d, d);
+}
+// 128 x 8 pixels per CTA, one column of 8 pixels per thread (8 running minima in registers); the axis values of 32
+// emitters at a time go through shared memory: one 64-bit load of dx2 and four 128-bit broadcast loads of dy2 per
+// eight distance tests.
+__global__ void __launch_bounds__(128) nearest_emitter_kernel(int Nx, int Ny, int M, const double *__restrict__ dx2,
+                                                              const double *__restrict__ dy2, int *__restrict__ owner) {
+    __shared__ double sx[32][128];
+    __shared__ __align__(16) double sy[32][8];
+    const int lx = threadIdx.x;
+    const int x0 = blockIdx.x * 128, y0 = blockIdx.y * 8;
+    int best[8];
+    double bd[8];
+#pragma unroll
+    for (int r = 0; r < 8; ++r) { best[r] = 0; bd[r] = 0.0; }
+    for (int e0 = 0; e0 < M; e0 += 32) {
+        __syncthreads();
+        for (int l = threadIdx.x; l < 32 * 128; l += 128) {
+            const int k = l / 128, c = l % 128;
+            sx[k][c] = (e0 + k < M && x0 + c < Nx) ? dx2[(size_t)(e0 + k) * Nx + x0 + c] : 0.0;
+        }
+        for (int l = threadIdx.x; l < 32 * 8; l += 128) {
+            const int k = l / 8, c = l % 8;
+            sy[k][c] = (e0 + k < M && y0 + c < Ny) ? dy2[(size_t)(e0 + k) * Ny + y0 + c] : 0.0;
+        }
+        __syncthreads();
+        const int ne = min(32, M - e0);
+        for (int k = 0; k < ne; ++k) {
+            const double ax = sx[k][lx];
+            const double2 *yp = reinterpret_cast<const double2 *>(sy[k]);
+#pragma unroll
+            for (int h = 0; h < 4; ++h) {
+                const double2 y2 = yp[h];
+                const double da = __dadd_rn(ax, y2.x), db = __dadd_rn(ax, y2.y);
+                if ((e0 + k) == 0 || da < bd[2 * h]) { bd[2 * h] = da; best[2 * h] = e0 + k; }
+                if ((e0 + k) == 0 || db < bd[2 * h + 1]) { bd[2 * h + 1] = db; best[2 * h + 1] = e0 + k; }
+            }
+        }
     }
-    owner[(size_t)y * Nx + x] = best;
+    if (x0 + lx < Nx) {
+#pragma unroll
+        for (int r = 0; r < 8; ++r)
+            if (y0 + r < Ny) owner[(size_t)(y0 + r) * Nx + x0 + lx] = best[r];
+    }
 }
 
 // Step 2: image[r] = sum over the T x T taps t of S[r - (t - T/2)] psf[owner[r - (t - T/2)]][t] (periodic).
-// A CTA computes a 32 x 8 patch; the (32 + T - 1) x (8 + T - 1) halo of S and owner sits in shared memory.
+// A CTA computes a 32 x 8 patch; the (32 + T - 1) x (8 + T - 1) halo of S and owner sits in shared memory.  The
+// owner map is piecewise constant, so a halo sees only a few emitters: their tiles are staged in shared memory too
+// (up to K of them, found with a small hash set) and the inner loop is three shared-memory loads and one FFMA per
+// tap; a halo with more than K emitters (cells much smaller than the tiles) gathers the tile values from global memory.
 __global__ void __launch_bounds__(256) image_formation_kernel(const float *__restrict__ S, const int *__restrict__ owner, int Nx, int Ny,
-                                                              const float *__restrict__ psf, int T, float *__restrict__ image) {
+                                                              const float *__restrict__ psf, int T, int K, float *__restrict__ image) {
     extern __shared__ float sm_if[];
-    const int HW = 32 + T - 1, HH = 8 + T - 1;
+    __shared__ int tab[64], slot_of[64], list[16], cnt, overflow;
+    const int HW = 32 + T - 1, HH = 8 + T - 1, TT = T * T;
     float *sS = sm_if;
     int *sO = reinterpret_cast<int *>(sm_if + HW * HH);
+    float *sP = sm_if + 2 * HW * HH;
     const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 8;
     // halo origin: source pixel r' = r - (t - T/2) ranges over [r - (T - 1 - T/2), r + T/2]
     const int hx0 = x0 - (T - 1 - T / 2), hy0 = y0 - (T - 1 - T / 2);
+    if (threadIdx.x < 64) tab[threadIdx.x] = -1;
+    if (threadIdx.x == 0) { cnt = 0; overflow = 0; }
     for (int i = threadIdx.x; i < HW * HH; i += 256) {
         const int hy = i / HW, hx = i - hy * HW;
         const int sx = ((hx0 + hx) % Nx + Nx) % Nx, sy = ((hy0 + hy) % Ny + Ny) % Ny;
@@ -208,16 +258,57 @@ __global__ void __launch_bounds__(256) image_formation_kernel(const float *__res
         sO[i] = owner[(size_t)sy * Nx + sx];
     }
     __syncthreads();
+    // the set of emitters in the halo
+    for (int i = threadIdx.x; i < HW * HH; i += 256) {
+        const int o = sO[i];
+        int h = o & 63, tries = 0;
+        for (; tries < 64; ++tries) {
+            const int prev = atomicCAS(&tab[h], -1, o);
+            if (prev == -1 || prev == o) break;
+            h = (h + 1) & 63;
+        }
+        if (tries == 64) overflow = 1;
+    }
+    __syncthreads();
+    if (threadIdx.x < 64 && tab[threadIdx.x] >= 0) {
+        const int sl = atomicAdd(&cnt, 1);
+        slot_of[threadIdx.x] = sl;
+        if (sl < K) list[sl] = tab[threadIdx.x];
+    }
+    __syncthreads();
+    const bool staged = !overflow && cnt <= K;
+    if (staged) {
+        const int n = cnt;
+        for (int i = threadIdx.x; i < n * TT; i += 256) {
+            const int sl = i / TT;
+            sP[i] = psf[(size_t)list[sl] * TT + (i - sl * TT)];
+        }
+        for (int i = threadIdx.x; i < HW * HH; i += 256) {
+            const int o = sO[i];
+            int h = o & 63;
+            while (tab[h] != o) h = (h + 1) & 63;
+            sO[i] = slot_of[h] * TT;
+        }
+    }
+    __syncthreads();
     const int lx = threadIdx.x % 32, ly = threadIdx.x / 32;
     const int x = x0 + lx, y = y0 + ly;
     if (x >= Nx || y >= Ny) return;
     float acc = 0.f;
-    for (int ty = 0; ty < T; ++ty)
-        for (int tx = 0; tx < T; ++tx) {
-            // r' = r - (t - T/2)  ->  halo index r' - h0 = l + (T - 1 - T/2) - (t - T/2) = l + T - 1 - t
-            const int hi = (ly + T - 1 - ty) * HW + (lx + T - 1 - tx);
-            acc = fmaf(sS[hi], __ldg(psf + ((size_t)sO[hi] * T + ty) * T + tx), acc);
+    if (staged) {
+        for (int ty = 0; ty < T; ++ty) {
+            const int hrow = (ly + T - 1 - ty) * HW + lx + T - 1, trow = ty * T;
+#pragma unroll 4
+            for (int tx = 0; tx < T; ++tx) acc = fmaf(sS[hrow - tx], sP[sO[hrow - tx] + trow + tx], acc);
         }
+    } else {
+        for (int ty = 0; ty < T; ++ty)
+            for (int tx = 0; tx < T; ++tx) {
+                // r' = r - (t - T/2)  ->  halo index r' - h0 = l + (T - 1 - T/2) - (t - T/2) = l + T - 1 - t
+                const int hi = (ly + T - 1 - ty) * HW + (lx + T - 1 - tx);
+                acc = fmaf(sS[hi], __ldg(psf + ((size_t)sO[hi] * T + ty) * T + tx), acc);
+            }
+    }
     image[(size_t)y * Nx + x] = acc;
 }
 
