@@ -375,6 +375,17 @@ def run_ours(args):
     }
     if clocks is not None:
         result["clocks"] = clocks
+    if rank == 0:
+        # fingerprints of the seeded inputs: the emitter arrays / initial fields in full, the dn volume by its
+        # first and last slice (hashing 4 GiB would take longer than the measurement)
+        import hashlib
+        sha = lambda a: hashlib.sha256(np.ascontiguousarray(a).tobytes()).hexdigest()[:16]
+        fp = {"dn_first_slice": sha(dn[0].cpu().numpy()), "dn_last_slice": sha(dn[-1].cpu().numpy())}
+        if em is not None:
+            fp["emitters"] = sha(np.concatenate([t.numpy().ravel() for t in em]))
+        else:
+            fp["field"] = sha(f0)
+        result["config"]["inputs_sha256_16"] = fp
 
     # ---- roofline of the dominant kernel (the persistent BPM kernel, one launch per propagation) ----
     hbm_b, l2_b, flop = algorithmic_per_step(w)
