@@ -338,7 +338,8 @@ __device__ __forceinline__ void run_phase8(const KParams &K, const Phase16 &d, c
                     for (int cc = 1; cc < P; ++cc)
                         v[jp * P + cc] = cmul_s<S2>(v[jp * P + cc], sm_twc[(cc - 1) * kL + tm.q(jp)]);
                 }
-                tm.sync();                                  // every read of the first exchange is done
+                // (no barrier here: a thread writes exactly the slots it read in the first exchange, and nobody
+                // else touches them in between)
 #pragma unroll
                 for (int jp = 0; jp < JP; ++jp)
 #pragma unroll
