@@ -521,18 +521,26 @@ def run_trace(args):
         bb.propagate(field, dn, w.dx, w.dz, w.lam, w.n0, intensity=inten, nref=nref)
         torch.cuda.synchronize()
     bb.probe_trace(None)
-    t = buf.cpu().numpy().astype(np.float64)
+    kernel = bb.last_kernel()
+    cluster = "bpmc_kernel" in kernel                         # grid = one cluster: the stamps of its CTAs come first
+    if cluster:
+        grid = int(kernel.split("<")[1].split(",")[2])
+    t = buf.cpu().numpy().astype(np.float64).reshape(-1)[: phases * grid * 6].reshape(phases, grid, 6)
     if not t[1:-1, :, 4].all():
         raise SystemExit("no trace recorded: this shape / batch does not run the traced kernel")
     # SM cycles per microsecond from the global timer (ns) at release of consecutive phases
     cyc_per_us = np.median((t[2:-1, :, 4] - t[1:-2, :, 4]) / np.maximum(t[2:-1, :, 5] - t[1:-2, :, 5], 1.0)) * 1e3
-    out = {"workload": w.name, "z_steps": w.Nz, "sm_cycles_per_us": cyc_per_us, "unit": "us (median over CTAs and steps)"}
+    out = {"workload": w.name, "z_steps": w.Nz, "kernel": kernel, "sm_cycles_per_us": cyc_per_us,
+           "unit": "us (median over CTAs and steps)"}
+    # grid kernels: work / barrier arrive / staging of the next factors / barrier wait;
+    # cluster kernel: transforms / send to the owners' shared memory / arrive + staging / wait
+    names = ("transforms", "send", "staging", "wait") if cluster else ("work", "arrive", "staging", "wait")
     for name, sel in (("row_phase", slice(2, phases - 1, 2)), ("column_phase", slice(1, phases - 1, 2))):
         p = t[sel]
-        seg = {"work": p[:, :, 1] - p[:, :, 0], "arrive": p[:, :, 2] - p[:, :, 1],
-               "staging": p[:, :, 3] - p[:, :, 2], "wait": p[:, :, 4] - p[:, :, 3], "total": p[:, :, 4] - p[:, :, 0]}
+        seg = {names[i]: p[:, :, i + 1] - p[:, :, i] for i in range(4)}
+        seg["total"] = p[:, :, 4] - p[:, :, 0]
         out[name] = {k: float(np.median(v) / cyc_per_us) for k, v in seg.items()}
-        out[name]["work_max_over_ctas"] = float(np.median(seg["work"].max(axis=1)) / cyc_per_us)
+        out[name][names[0] + "_max_over_ctas"] = float(np.median(seg[names[0]].max(axis=1)) / cyc_per_us)
     rel = t[1:-1, :, 5].max(axis=1)
     out["us_per_z_step"] = float(np.median(rel[2:] - rel[:-2]) * 1e-3)
     print(json.dumps(out))

@@ -86,6 +86,8 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
                 obj = os.path.join(OBJ, "bb_inst8_px%d_cw%d_b%d.o" % (px, cw, bt))
                 jobs.append((obj, [nvcc, *NVCC_FLAGS, "-DBB_PX=%d" % px, "-DBB_CW=%d" % cw, "-DBB_BATCH=%d" % bt, "-c",
                                    os.path.join(CSRC, "bb_inst8.cu"), "-o", obj]))
+    obj_c = os.path.join(OBJ, "bb_instc.o")
+    jobs.append((obj_c, [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, "bb_instc.cu"), "-o", obj_c]))
     obj_api = os.path.join(OBJ, "bb_api.o")
     jobs.append((obj_api, [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, "bb_api.cu"), "-o", obj_api]))
     obj_probe = os.path.join(OBJ, "bb_probe.o")

@@ -75,6 +75,10 @@ struct Plan {
     bool k8 = false;               // 8-point-thread kernel available for this shape
     bool k32 = false;              // 32-point-thread kernel (all shapes up to 1024; transform programs)
     bool force_k8 = false;         // BB_USE_K8=1 when the plan was made
+    int kc_cs = 0;                 // cluster kernel (grids up to 256^2): CTAs per cluster, 0 = not available
+    int kc_mode = 1;               // ... exchange: 1 bulk copies counted on mbarriers, 0 remote stores + cluster barriers (BB_KC_MODE)
+    int kc_pt = 8;                 // ... points per thread: 16 on 256 x 256 (BB_KC_PT=8: the 8-point form there too)
+    bool kc_force = false;         // BB_KC_FORCE=1: use it on 256 x 256 as well
     // diagnostic switches, read once when the plan is made (bb_shutdown + a new call re-reads them)
     bool env_notma = false, env_noprune = false;
     int env_cw = 0;                // BB_K16_CW: 4 or 8, 0 = automatic
@@ -223,6 +227,18 @@ int get_plan(int Nx, int Ny, Plan **out) {
         p->k32 = true;
     }
     if (!p->k32 && !p->k8) { return fail(BB_ERR_UNSUPPORTED_SHAPE, "no kernel for Nx = %d, Ny = %d", Nx, Ny); }
+    if (bb::kernelc_supports(Nx, Ny) && !getenv("BB_DISABLE_KC") && !getenv("BB_USE_K8")) {
+        // the largest cluster the device schedules: 16 CTAs (non-portable size) halve the per-CTA share of the exchange
+        p->kc_mode = getenv("BB_KC_MODE") ? (atoi(getenv("BB_KC_MODE")) != 0) : 1;
+        p->kc_pt = Nx == 256 && Ny == 256 && !(getenv("BB_KC_PT") && atoi(getenv("BB_KC_PT")) == 8) ? 16 : 8;
+        p->kc_force = getenv("BB_KC_FORCE") != nullptr;
+        const int want = getenv("BB_KC_CS") ? atoi(getenv("BB_KC_CS")) : 0;
+        for (int cs : {16, 8}) {
+            if (want && cs != want) continue;
+            if (bb::kernelc_prepare(Nx, Ny, cs, p->kc_mode, p->kc_pt) != 0) { (void)cudaGetLastError(); continue; }
+            if (bb::kernelc_max_clusters(Nx, Ny, cs, p->kc_mode, p->kc_pt) >= 1) { p->kc_cs = cs; break; }
+        }
+    }
     p->grid = sms;
     p->env_notma = getenv("BB_K16_NOTMA") != nullptr;
     p->env_noprune = getenv("BB_K16_NOPRUNE") != nullptr;
@@ -426,6 +442,17 @@ bool use_k16(const Plan *p, int B) {
     return B == 1 || (long long)rows * p->Nx <= 8192;
 }
 
+// The cluster kernel (bb_kernelsc.cuh: one cluster per field, the field in distributed shared memory) takes every
+// grid with a 128-point side that it supports: 2.5 - 5 x faster than the grid kernels there, single fields and
+// batches (profiles/r02_cluster_kernel.md).  On 256 x 256 it only ties with the 16-point-thread grid kernel for a
+// single field (both 7.8 us per step: the exchange is bound by the 16 CTAs' distributed-shared-memory bandwidth) and
+// loses for batches of 16 and more, so it is not used there unless BB_KC_FORCE=1 (tests, measurements).
+bool use_kc(const Plan *p, int B) {
+    (void)B;
+    if (p->kc_cs == 0) return false;
+    return p->kc_force || p->Nx == 128 || p->Ny == 128;
+}
+
 int batch_warps(int B) {
     int bw = 1;
     while (bw < B && bw < bb::kWarps) bw <<= 1;
@@ -450,21 +477,26 @@ int launch_steps(Plan *p, cf *field, const float *dn, float *inten, long long in
     P.flags = flags & 3u;
     P.backward = (flags & BB_BACKWARD) ? 1 : 0;
     P.noscreen = (flags & BB_HOMOGENEOUS) ? 1 : 0;
-    const bool k8 = use_k8(p, B), k16 = use_k16(p, B);
-    if (!k8 && !k16 && !p->k32) return fail(BB_ERR_UNSUPPORTED_SHAPE, "no kernel for Nx = %d, Ny = %d, batch = %d", p->Nx, p->Ny, B);
+    const bool kc = use_kc(p, B);
+    const bool k8 = !kc && use_k8(p, B), k16 = !kc && use_k16(p, B);
+    if (!kc && !k8 && !k16 && !p->k32) return fail(BB_ERR_UNSUPPORTED_SHAPE, "no kernel for Nx = %d, Ny = %d, batch = %d", p->Nx, p->Ny, B);
     if (k16 || k8) P.use_tma = !p->env_notma && make_field_tmap(&P.tmap, field, p->Nx, p->Ny, B, p->cw4 ? 4 : 8) ? 1 : 0;
-    if (g_trace && g_trace_dev == p->device && (k16 || k8) && 2 * Nz_total + 1 <= g_trace_phases) { P.trace = g_trace; P.trace_p0 = 0; }
+    if (g_trace && g_trace_dev == p->device && (kc || k16 || k8) && 2 * Nz_total + 1 <= g_trace_phases) { P.trace = g_trace; P.trace_p0 = 0; }
     snprintf(g_last_kernel, sizeof g_last_kernel, k8 ? "bb::bpm8_kernel<%d,%d,%d,%s>" : k16 ? "bb::bpm16_kernel<%d,%d,%d,%s>" : "bb::bpm_kernel<%d,%d,%d>",
              k8 || k16 ? p->Nx / 256 : p->Nx / 32, k8 || k16 ? p->Ny / 256 : p->Ny / 32, k8 || k16 ? (p->cw4 ? 4 : 8) : 8,
              B > 1 ? "true" : "false");
+    if (kc) snprintf(g_last_kernel, sizeof g_last_kernel, "bb::bpmc_kernel<%d,%d,%d,%d,%d>", p->Nx, p->Ny, p->kc_cs, p->kc_mode, p->kc_pt);
     auto launch = [&](bool coop) {
-        return k8 ? bb::kernel8_launch(p->Nx, p->Ny, P, p->grid, coop, s)
+        return kc ? bb::kernelc_launch(p->Nx, p->Ny, p->kc_cs, p->kc_mode, p->kc_pt, P, B, s)
+             : k8 ? bb::kernel8_launch(p->Nx, p->Ny, P, p->grid, coop, s)
                   : k16 ? bb::kernel16_launch(p->Nx, p->Ny, P, p->run_grid > 0 ? p->run_grid : p->grid, coop, s)
                         : bb::kernel_launch(p->Nx, p->Ny, P, p->grid, coop, s);
     };
     // steps [j0, j1): forward = column phases j0 .. j1-1 and the row phases after them (plus row phase 0);
     // backward = row / column phases Nz-j1 .. Nz-1-j0 in that order (plus the closing row phase Nz)
     int p0 = (j0 == 0) ? 0 : 2 * j0 + 1, p1 = 2 * j1 + 1;
+    if (kc && B > 1 && inten && !(flags & BB_INTENSITY_PER_FIELD) && !(flags & BB_ACCUMULATE))
+        BB_CUDA(cudaMemsetAsync(inten, 0, (size_t)(j1 - j0) * p->Nx * p->Ny * sizeof(float), s));   // the clusters add into it
     if (flags & BB_BACKWARD) { p0 = 2 * (Nz_total - j1); p1 = 2 * (Nz_total - j0) + (j0 == 0 ? 1 : 0); }
     if (flags & BB_LAUNCH_PER_PHASE) {
         for (int ph = p0; ph < p1; ++ph) {
@@ -721,7 +753,7 @@ int propagate_impl(void *field, const float *dn, int Nx, int Ny, int Nz, float d
     // A batch the batch variant of the 16-point-thread kernel cannot take (the screen factors of a CTA's rows
     // must fit one buffer) runs field by field on its single-field variant -- faster than the 32-point-thread
     // kernel, and the only way on a grid with a 2048-point side; dn is then read once per field.
-    if (B > 1 && p->k16 && !use_k16(p, B) && !use_k8(p, B)) {
+    if (B > 1 && p->k16 && !use_k16(p, B) && !use_k8(p, B) && !use_kc(p, B)) {
         const size_t npx1 = (size_t)Nx * Ny;
         for (int b = 0; b < B; ++b) {
             bb_opts o = *opts;
@@ -884,7 +916,7 @@ int propagate_host_impl(void *field_host, const float *dn_host, int Nx, int Ny, 
     if (rc) return rc;
     DeviceCtx &ctx = device_ctx();
     const float *nref = opts ? opts->nref : nullptr;
-    if (B > 1 && p->k16 && !use_k16(p, B) && !use_k8(p, B)) {       // as in propagate_impl: field by field
+    if (B > 1 && p->k16 && !use_k16(p, B) && !use_k8(p, B) && !use_kc(p, B)) {   // as in propagate_impl: field by field
         const size_t npx1 = (size_t)Nx * Ny;
         for (int b = 0; b < B; ++b) {
             bb_opts o = *opts;

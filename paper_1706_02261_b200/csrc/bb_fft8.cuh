@@ -58,8 +58,10 @@ __device__ __forceinline__ cf mul_w16(cf a) { return mul_w32x<2 * M, SIGN>(a); }
 __device__ __forceinline__ cf fma2c(float s, cf a, cf b) {      // s a + b, per component
     return up2(fma2(pk2(s, s), pk2(a.x, a.y), pk2(b.x, b.y)));
 }
+// the value of the other lane of the pair (lane ^ X; X = 16: one pair per sub-line index t of a warp)
+template <int X = 16>
 __device__ __forceinline__ cf shfl16(cf a) {
-    return make_float2(__shfl_xor_sync(0xFFFFFFFFu, a.x, 16), __shfl_xor_sync(0xFFFFFFFFu, a.y, 16));
+    return make_float2(__shfl_xor_sync(0xFFFFFFFFu, a.x, X), __shfl_xor_sync(0xFFFFFFFFu, a.y, X));
 }
 
 // Radix-8 DFT, natural order in, out[k] = X[(k + 4 r) mod 8] with r = 0 for s = +1, r = 1 for s = -1
@@ -111,7 +113,7 @@ __device__ __forceinline__ void dft8_rot_in(cf (&v)[8], float s) {
 // w = exp(SIGN 2 pi i / 16).  Lane 1 produces E1 rotated by four (dft8_rot_out) and twiddled, so that
 // both lanes keep registers 0..3 and trade registers 4..7 (lane 1 sends its half negated):
 //   out[j] = own[j] - s recv[j],   out[4 + j] = s own[j] + recv[j].
-template <int SIGN>
+template <int SIGN, int X = 16>
 __device__ __forceinline__ void pair16_dit(cf (&v)[8], int h, float s) {
     dft8_rot_out<SIGN>(v, s);
     if (h) {
@@ -120,7 +122,7 @@ __device__ __forceinline__ void pair16_dit(cf (&v)[8], int h, float s) {
     }
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
-        const cf r = shfl16(v[4 + j]);
+        const cf r = shfl16<X>(v[4 + j]);
         const cf own = v[j];
         v[j] = fma2c(-s, r, own);
         v[4 + j] = fma2c(s, own, r);
@@ -131,14 +133,14 @@ __device__ __forceinline__ void pair16_dit(cf (&v)[8], int h, float s) {
 //   u[m] = x[m] + x[m + 8], d[m] = (x[m] - x[m + 8]) w^m, m < 8;  X[2k] = DFT8(u)[k], X[2k + 1] = DFT8(d)[k].
 // Lane h holds m = 4 h + j: it keeps the half its own output parity needs (lane 0: u, lane 1: the raw
 // difference), sends the other, and lane 1 runs its radix-8 on inputs rotated by four (dft8_rot_in).
-template <int SIGN>
+template <int SIGN, int X = 16>
 __device__ __forceinline__ void pair16_dif(cf (&v)[8], int h, float s) {
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         const cf keep = fma2c(s, v[4 + j], v[j]);
         const cf send = fma2c(-s, v[4 + j], v[j]);
         v[j] = keep;
-        v[4 + j] = shfl16(send);
+        v[4 + j] = shfl16<X>(send);
     }
     if (h) {   // register i holds the raw difference of m = (i + 4) mod 8
         v[0] = mul_w16<4, SIGN>(v[0]); v[1] = mul_w16<5, SIGN>(v[1]); v[2] = mul_w16<6, SIGN>(v[2]); v[3] = mul_w16<7, SIGN>(v[3]);

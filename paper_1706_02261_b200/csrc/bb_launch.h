@@ -55,4 +55,10 @@ int kernel8_prepare(int Nx, int Ny);
 int kernel8_blocks_per_sm(int Nx, int Ny);
 cudaError_t kernel8_launch(int Nx, int Ny, const KParams &P, int grid, bool coop, cudaStream_t s);
 
+// Cluster kernel for small grids (bb_kernelsc.cuh; bb_instc.cu): one cluster of `cs` CTAs per field.
+bool kernelc_supports(int Nx, int Ny);
+int kernelc_prepare(int Nx, int Ny, int cs, int mode, int pt);        // returns a cudaError_t value
+int kernelc_max_clusters(int Nx, int Ny, int cs, int mode, int pt);   // clusters the device holds at once; 0: cannot be scheduled
+cudaError_t kernelc_launch(int Nx, int Ny, int cs, int mode, int pt, const KParams &P, int nclusters, cudaStream_t s);
+
 }  // namespace bb
