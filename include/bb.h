@@ -98,12 +98,18 @@ int bb_propagate(void *field, const float *dn_volume, int Nx, int Ny, int Nz,
 
 /* Same with options (batch, adapted n_ref, accumulate / per-field intensity, backward, homogeneous,
  * stream).  opts may be NULL.  Kernel selection (results do not depend on it beyond rounding): grids
+ * with both sides in {128, 256} and at least one side of 128 run the cluster kernel -- one thread-block
+ * cluster of 16 CTAs (8 if the device cannot place 16) per field, the field resident in the cluster's
+ * distributed shared memory for the whole call, dn and the intensity the only per-step global traffic;
+ * batches take one cluster per field, and a summed batch intensity is then added up with global atomics
+ * into slices the call zeroes first (BB_KC_FORCE=1 in the environment: 256 x 256 as well; BB_DISABLE_KC=1:
+ * never) -- other grids
  * with sides in {256, 512, 1024, 2048} run the 16-point-thread kernel -- for a batch only while the screen
  * factors of a CTA's rows fit its buffer, ceil(Ny / SMs) * Nx <= 8192; a larger batch runs field by field
  * on the single-field variant (dn is then read once per field) -- everything else the 32-point-thread kernel
  * (sides up to 1024).  The 8-point-thread kernel runs the transforms of bb_fft2 / bb_multiplex_* on grids with a 2048-point
  * side and, with BB_USE_K8=1 in the environment, propagations.  The summed intensity of a
- * batch is accumulated with shared-memory atomics: its summation order, hence its last bits, can
+ * batch is accumulated with atomics (shared memory, or global memory in the cluster kernel): its summation order, hence its last bits, can
  * differ between runs (tolerance contract: relative L2 <= 1e-4 against the definition). */
 int bb_propagate_ex(void *field, const float *dn_volume, int Nx, int Ny, int Nz,
                     float dx, float dz, float lambda, float n0, float *intensity_out,

@@ -178,7 +178,7 @@ __device__ __forceinline__ void screen_to_pw(float (&x)[PT], float pa, float pb,
             pw[i * NT] = make_float2(c, s);
         }
     } else {
-#pragma unroll 2
+#pragma unroll      // (a rolled loop would index x[] dynamically and put the thread's dn values in local memory)
         for (int i = 0; i < PT; ++i) {
             float s, c;
             screen_sincos(x[i], s, c);
@@ -270,11 +270,13 @@ __global__ void __launch_bounds__(SmemC<NX, NY, CS, PT>::NT, 1) bpmc_kernel(cons
     auto send_tiles = [&](cf *own, cf *theirs, int which) {
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // my writes, before the copy engine reads them
         __syncthreads();
-        // one copy per tile, issued by lane 0 of the warps in turn (the copies of one warp are issued one after the other)
-        if ((tid & 31) == 0)
-            for (int t = tid >> 5; t < CS; t += NT / 32)
-                bulk_to_cta(dsmem_addr(theirs + rank * TILE, (unsigned)t), own + t * TILE, kTileBytes,
-                            dsmem_addr(sm_mbar + which, (unsigned)t));
+        // one copy per tile, spread over the warps (a warp issues its copies one after the other: ~30 ns each from
+        // different lanes, ~70 ns each from a loop in one lane)
+        constexpr int NW = NT / 32, TPW = (CS + NW - 1) / NW;
+        const int t = (tid >> 5) * TPW + (tid & 31);
+        if ((tid & 31) < TPW && t < CS)
+            bulk_to_cta(dsmem_addr(theirs + rank * TILE, (unsigned)t), own + t * TILE, kTileBytes,
+                        dsmem_addr(sm_mbar + which, (unsigned)t));
     };
 
     Phase16 d = decode_phase16(P, P.p0);
