@@ -165,22 +165,25 @@ def test_forward_then_backward_returns_the_input(kc_env):
     assert rel_l2(d.cpu().numpy(), f0) < 2e-5
 
 
-def test_host_buffers_in_several_chunks(oracle_mod, kc_env):
+@pytest.mark.parametrize("backward", [False, True])
+def test_host_buffers_in_several_chunks(oracle_mod, kc_env, backward):
     """bb_propagate_host cuts 128^2 x 1100 slices into chunks of 512: every launch but the first starts from the
-    field in global memory half way through a step, every launch but the last leaves it there.  Same bits as the
-    one-launch device run."""
+    field in global memory half way through a step, every launch but the last leaves it there (forward: launches
+    start and end on row phases; backward: they end on column phases).  Same bits as the one-launch device run."""
     bb = kc_env()
     Nz = 1100
     w, dn, f0, nref = problem(oracle_mod, 128, 128, Nz, 1, seed=2, slab=64)
+    flags = bb.BACKWARD if backward else 0
     d = torch.from_numpy(f0.copy()).cuda()
     I = torch.empty(dn.shape, device="cuda")
-    bb.propagate(d, dn.cuda(), w.dx, w.dz, w.lam, w.n0, intensity=I, nref=nref)
+    bb.propagate(d, dn.cuda(), w.dx, w.dz, w.lam, w.n0, intensity=I, nref=nref, flags=flags)
     assert "bpmc_kernel" in bb.last_kernel()
     fh = torch.from_numpy(f0.copy()).pin_memory()
     Ih = torch.empty(dn.shape).pin_memory()
-    bb.propagate(fh, dn.pin_memory(), w.dx, w.dz, w.lam, w.n0, intensity=Ih, nref=nref)
+    bb.propagate(fh, dn.pin_memory(), w.dx, w.dz, w.lam, w.n0, intensity=Ih, nref=nref, flags=flags)
     assert torch.equal(fh, d.cpu()) and torch.equal(Ih, I.cpu())
-    uo, Io = oracle_mod.propagate(f0[0], dn.numpy(), w.dx, w.dz, w.lam, w.n0, nref=nref)
+    ofn = oracle_mod.propagate_backward if backward else oracle_mod.propagate
+    uo, Io = ofn(f0[0], dn.numpy(), w.dx, w.dz, w.lam, w.n0, nref=nref)
     assert rel_l2(fh.numpy()[0], uo) < 1e-4 and rel_l2(Ih.numpy(), Io) < 1e-4
 
 
