@@ -138,6 +138,35 @@ int bb_nref_from_dn(const float *dn_volume, int Nx, int Ny, int Nz, float n0, in
                     float *nref_out_host, void *stream);
 
 /*
+ * bb_nref_from_dn_static -- the same n_ref[j] (reading A3; same arithmetic, results
+ * equal to bb_nref_from_dn's to one float32 ulp) for callers that must not allocate.  bb_nref_from_dn
+ * grows a device workspace with cudaFree + cudaMalloc and fills a host vector.  That is wrong for a
+ * pipeline that works out n_ref of the next volume on a side stream while a propagation runs (cudaMalloc
+ * and cudaFree wait for the whole device, so the propagation stalls), and for a process whose own
+ * allocator already holds nearly all device memory (a raw cudaMalloc then fails).  This entry point makes
+ * no cudaMalloc / cudaFree / host allocation and no copy: two kernel launches on `stream`, returning
+ * without waiting.
+ *   dn_volume   DEVICE float[Nz][Ny][Nx] (any Nx, Ny >= 1)
+ *   nref_out    DEVICE float[Nz], caller-owned -- not the HOST array of bb_nref_from_dn; copy it to the
+ *               host yourself (bb_opts.nref wants it there), into memory you already own
+ * Scratch: Nz x 16 doubles of per-slice partial sums in a fixed array inside the library's device
+ * image, BB_STATIC_MAX_NZ slices deep = 512 KiB, resident on every GPU whose context loads this library
+ * until the process exits.  Nz > BB_STATIC_MAX_NZ returns BB_ERR_INVALID_ARG (message names the limit);
+ * split deeper volumes along z on slab boundaries, or use bb_nref_from_dn.
+ * First call on each device: looks up the array's device address (cudaGetSymbolAddress, once per device,
+ * cached; that device must be current, as for every call here).  Make that first call outside any stream
+ * capture.
+ * All calls on one device share the array.  Nothing needs to start at zero: each call overwrites every
+ * element it later reads, so the previous call's contents never show.  But two calls that can overlap on
+ * the GPU (different streams without an event between them) race on it and both results are garbage; on
+ * one stream they are ordered and safe.
+ */
+#define BB_STATIC_MAX_NZ 4096
+int bb_nref_from_dn_static(const float *dn_volume, int Nx, int Ny, int Nz, float n0, int slab,
+                           float *nref_out, void *stream);
+int bb_static_max_nz(void);             /* BB_STATIC_MAX_NZ of the loaded library */
+
+/*
  * bb_multiplex_psf -- north_star: "bb_multiplex_psf(emitter_positions, NA, ...)"; PAPER.md
  * line 21 ("sets of 100s to 1000s of mutually independent ... PSFs ... within single, highly
  * multiplexed simulations") and line 29 ("multiplexed diffraction-limited point-sources").

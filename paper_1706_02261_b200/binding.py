@@ -24,7 +24,7 @@ HOMOGENEOUS = 16
 EXPORTS = ("bb_propagate", "bb_propagate_ex", "bb_propagate_host", "bb_nref_from_dn",
            "bb_multiplex_psf", "bb_fft2", "bb_propagator_table", "bb_last_error", "bb_version",
            "bb_shutdown", "bb_launch_count", "bb_device_status", "bb_probe_l2_bandwidth", "bb_probe_fp32", "bb_probe_trace",
-           "bb_last_kernel", "bb_multiplex_annular", "bb_lightsheet", "bb_refocus", "bb_extract_tiles", "bb_image_formation")
+           "bb_last_kernel", "bb_nref_from_dn_static", "bb_static_max_nz", "bb_multiplex_annular", "bb_lightsheet", "bb_refocus", "bb_extract_tiles", "bb_image_formation")
 
 STATUS_NAMES = {0: "BB_OK", 1: "BB_ERR_INVALID_ARG", 2: "BB_ERR_UNSUPPORTED_SHAPE", 3: "BB_ERR_CUDA",
                 4: "BB_ERR_OOM", 5: "BB_ERR_ARCH", 6: "BB_ERR_INTERNAL"}
@@ -60,6 +60,7 @@ def load() -> ctypes.CDLL:
     lib.bb_propagate_ex.argtypes = [vp, vp, i, i, i, f, f, f, f, vp, ctypes.POINTER(_Opts)]
     lib.bb_propagate_host.argtypes = [vp, vp, i, i, i, f, f, f, f, vp, ctypes.POINTER(_Opts)]
     lib.bb_nref_from_dn.argtypes = [vp, i, i, i, f, i, fp, vp]
+    lib.bb_nref_from_dn_static.argtypes = [vp, i, i, i, f, i, vp, vp]
     lib.bb_multiplex_psf.argtypes = [vp, vp, vp, i, f, i, i, f, f, vp, vp]
     lib.bb_multiplex_annular.argtypes = [vp, vp, vp, i, f, f, i, i, f, f, vp, vp]
     lib.bb_lightsheet.argtypes = [i, i, f, f, f, f, f, vp, vp]
@@ -175,6 +176,26 @@ def nref_from_dn(dn: torch.Tensor, n0: float, slab: int, stream=None) -> torch.T
     with torch.cuda.device(dn.device):
         _check(lib.bb_nref_from_dn(ctypes.c_void_p(dn.data_ptr()), Nx, Ny, Nz, n0, slab, out, _stream_ptr(stream)))
     return torch.tensor(list(out), dtype=torch.float32)
+
+
+def static_max_nz() -> int:
+    return int(load().bb_static_max_nz())
+
+
+def nref_from_dn_static(dn: torch.Tensor, n0: float, slab: int, out: torch.Tensor, stream=None) -> torch.Tensor:
+    """``bb_nref_from_dn_static``: n_ref per slice into ``out``, a CUDA float32 tensor of Nz elements that
+    the CALLER supplies -- this wrapper creates no tensor, because the entry point exists for callers that
+    must not allocate (see ``include/bb.h``).  Asynchronous on ``stream``; at most ``static_max_nz()`` slices."""
+    lib = load()
+    _f32(dn, "dn")
+    _f32(out, "out")
+    Nz, Ny, Nx = dn.shape
+    if not dn.is_cuda or not out.is_cuda or out.device != dn.device or out.numel() != Nz:
+        raise TypeError("dn and out must be CUDA tensors on one device, out with Nz = %d elements" % Nz)
+    with torch.cuda.device(dn.device):
+        _check(lib.bb_nref_from_dn_static(ctypes.c_void_p(dn.data_ptr()), Nx, Ny, Nz, n0, slab,
+                                          ctypes.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+    return out
 
 
 def multiplex_psf(pos: torch.Tensor, phase: Optional[torch.Tensor], amp: Optional[torch.Tensor], NA: float,

@@ -92,6 +92,8 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
     jobs.append((obj_api, [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, "bb_api.cu"), "-o", obj_api]))
     obj_probe = os.path.join(OBJ, "bb_probe.o")
     jobs.append((obj_probe, [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, "bb_probe.cu"), "-o", obj_probe]))
+    obj_na = os.path.join(OBJ, "bb_noalloc.o")
+    jobs.append((obj_na, [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, "bb_noalloc.cu"), "-o", obj_na]))
     todo = [(o, c) for o, c in jobs if force or _stale(o, deps)]          # objects newer than every source are kept
     with concurrent.futures.ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
         for out in ex.map(lambda oc: _run(oc[1]), todo):

@@ -1180,3 +1180,13 @@ int bb_multiplex_annular(const float *pos, const float *phase, const float *amp,
 }
 
 }  // extern "C"
+
+// Hooks for the library's other translation units (bb_hooks.h).
+#include "bb_hooks.h"
+namespace bb {
+int report_error(int code, const char *message) { return fail(code, "%s", message); }
+void count_launches(unsigned n) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    g_launches += n;
+}
+}  // namespace bb

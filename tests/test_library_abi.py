@@ -109,6 +109,9 @@ def test_argument_checks_come_before_any_device_work(lib):
     assert lib.bb_multiplex_psf(fake, None, None, 0, 0.8, 128, 128, 0.1, 0.5, fake, None) == 1
     assert lib.bb_multiplex_psf(fake, None, None, 4, -0.8, 128, 128, 0.1, 0.5, fake, None) == 1
     assert lib.bb_nref_from_dn(None, 128, 128, 4, 1.33, 2, None, None) == 1
+    assert lib.bb_nref_from_dn_static(None, 128, 128, 4, 1.33, 2, fake, None) == 1
+    assert lib.bb_nref_from_dn_static(fake, 128, 128, lib.bb_static_max_nz() + 1, 1.33, 2, fake, None) == 1 \
+        and "BB_STATIC_MAX_NZ" in err()
     assert lib.bb_propagator_table(128, 128, 0.1, 0.1, 0.5, 1.33, None, None) == 1
 
 
