@@ -264,10 +264,13 @@ int bb_probe_l2_bandwidth(unsigned long long bytes, int iters, int mode, double 
 int bb_probe_fp32(int iters, int packed, double *tflops);
 /*
  * bb_probe_trace: timeline of the persistent kernel, for profiling only.  device_buf is a DEVICE
- * long long[phases][grid][6] (grid = SM count) or NULL to switch tracing off.  While set, every
- * single-field propagation of at most (phases - 1) / 2 steps on a 256/512/1024 grid records, per
- * phase and CTA, the SM clock at phase start, work done, barrier arrived, pointwise factors staged
- * and barrier released, and the global nanosecond timer at release.
+ * long long[phases][SM count][6] or NULL to switch tracing off.  While set, every propagation of at
+ * most (phases - 1) / 2 steps records, per phase and CTA (index = blockIdx.x, which must stay below the
+ * SM count), the SM clock at phase start, work done, barrier arrived, pointwise factors staged and
+ * barrier released, and the global nanosecond timer at release.  Traced: the 16- and 8-point-thread
+ * grid kernels (sides 256 .. 2048; grid <= SM count, single fields and batches) and the cluster kernel
+ * for a SINGLE field (a 128-point side; its grid is the cluster size, 8 or 16 CTAs).  A batch on the
+ * cluster kernel launches cluster size x B CTAs, more than the buffer has rows for, and is not traced.
  */
 int bb_probe_trace(long long *device_buf, int phases);
 

@@ -481,7 +481,9 @@ int launch_steps(Plan *p, cf *field, const float *dn, float *inten, long long in
     const bool k8 = !kc && use_k8(p, B), k16 = !kc && use_k16(p, B);
     if (!kc && !k8 && !k16 && !p->k32) return fail(BB_ERR_UNSUPPORTED_SHAPE, "no kernel for Nx = %d, Ny = %d, batch = %d", p->Nx, p->Ny, B);
     if (k16 || k8) P.use_tma = !p->env_notma && make_field_tmap(&P.tmap, field, p->Nx, p->Ny, B, p->cw4 ? 4 : 8) ? 1 : 0;
-    if (g_trace && g_trace_dev == p->device && (kc || k16 || k8) && 2 * Nz_total + 1 <= g_trace_phases) { P.trace = g_trace; P.trace_p0 = 0; }
+    // The trace buffer holds [phases][SM count][6] records.  The grid kernels never launch more CTAs than SMs; the cluster
+    // kernel launches kc_cs * B of them, which fits for a single field only (kc_cs <= 16), so batches there are not traced.
+    if (g_trace && g_trace_dev == p->device && ((kc && B == 1) || k16 || k8) && 2 * Nz_total + 1 <= g_trace_phases) { P.trace = g_trace; P.trace_p0 = 0; }
     snprintf(g_last_kernel, sizeof g_last_kernel, k8 ? "bb::bpm8_kernel<%d,%d,%d,%s>" : k16 ? "bb::bpm16_kernel<%d,%d,%d,%s>" : "bb::bpm_kernel<%d,%d,%d>",
              k8 || k16 ? p->Nx / 256 : p->Nx / 32, k8 || k16 ? p->Ny / 256 : p->Ny / 32, k8 || k16 ? (p->cw4 ? 4 : 8) : 8,
              B > 1 ? "true" : "false");
@@ -916,21 +918,12 @@ int propagate_host_impl(void *field_host, const float *dn_host, int Nx, int Ny, 
     if (rc) return rc;
     DeviceCtx &ctx = device_ctx();
     const float *nref = opts ? opts->nref : nullptr;
-    if (B > 1 && p->k16 && !use_k16(p, B) && !use_k8(p, B) && !use_kc(p, B)) {   // as in propagate_impl: field by field
-        const size_t npx1 = (size_t)Nx * Ny;
-        for (int b = 0; b < B; ++b) {
-            bb_opts o = *opts;
-            o.batch = 1;
-            o.flags = flags & ~BB_INTENSITY_PER_FIELD;
-            float *I = inten_host;
-            if (inten_host && (flags & BB_INTENSITY_PER_FIELD)) I = inten_host + (size_t)b * Nz * npx1;
-            else if (b > 0) o.flags |= BB_ACCUMULATE;
-            rc = propagate_host_impl((cf *)field_host + (size_t)b * npx1, dn_host, Nx, Ny, Nz, dx, dz, lambda, n0, I, &o);
-            if (rc) return rc;
-        }
-        return BB_OK;
-    }
-    choose_tile_width(p, B, Nz, dx, lambda, n0, nref);
+    // A batch the batch kernels cannot take runs field by field on the single-field kernel, as in propagate_impl --
+    // but inside the chunk loop below, one launch per field on the resident dn chunk, so that every dn chunk crosses
+    // PCIe once per call and the three streams keep running (not once per field with the streams drained in between).
+    const bool fbf = B > 1 && p->k16 && !use_k16(p, B) && !use_k8(p, B) && !use_kc(p, B);
+    const int LB = fbf ? 1 : B;                              // fields per launch
+    choose_tile_width(p, LB, Nz, dx, lambda, n0, nref);
     const size_t npx = (size_t)Nx * Ny;
     const bool per_field = (flags & BB_INTENSITY_PER_FIELD) != 0;
     const bool backward = (flags & BB_BACKWARD) != 0;
@@ -992,15 +985,23 @@ int propagate_host_impl(void *field_host, const float *dn_host, int Nx, int Ny, 
         int i = ia;
         while (i < ib) {
             if (i >= prepared) {
-                rc = prepare_steps(p, B, Nz, i, dx, dz, lambda, n0, nref, flags, s_run, h_tab, h_phase, &prepared);
+                rc = prepare_steps(p, LB, Nz, i, dx, dz, lambda, n0, nref, flags, s_run, h_tab, h_phase, &prepared);
                 if (rc || prepared <= i) { drain(); return rc ? rc : fail(BB_ERR_OOM, "propagator table cache too small"); }
             }
             const int ie = std::min(ib, prepared);
             const int ja = backward ? Nz - ie : i, jb = backward ? Nz - i : ie;    // the steps of this launch
-            rc = launch_steps(p, d_field, dn_b ? dn_b + (size_t)(ja - j0) * npx : nullptr,
-                              I_b ? I_b + (size_t)(ja - j0) * npx : nullptr, (long long)CZ * (long long)npx,
-                              B, Nz, ja, jb, phase_b, flags, s_run);
-            if (rc) { drain(); return rc; }
+            for (int b = 0; b < (fbf ? B : 1); ++b) {
+                float *I_l = I_b ? I_b + (size_t)(ja - j0) * npx : nullptr;
+                unsigned fl = flags;
+                if (fbf) {                                   // one field: its own volume, or added to the sum of the earlier ones
+                    fl &= ~(unsigned)BB_INTENSITY_PER_FIELD;
+                    if (per_field) { if (I_l) I_l += (size_t)b * CZ * npx; }
+                    else if (b > 0) fl |= BB_ACCUMULATE;
+                }
+                rc = launch_steps(p, d_field + (fbf ? (size_t)b * npx : 0), dn_b ? dn_b + (size_t)(ja - j0) * npx : nullptr,
+                                  I_l, (long long)CZ * (long long)npx, LB, Nz, ja, jb, phase_b, fl, s_run);
+                if (rc) { drain(); return rc; }
+            }
             i = ie;
         }
         BB_TRY(cudaEventRecord(ev_run[c], s_run));

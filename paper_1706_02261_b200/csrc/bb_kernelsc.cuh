@@ -256,20 +256,23 @@ __global__ void __launch_bounds__(SmemC<NX, NY, CS, PT>::NT, 1) bpmc_kernel(cons
     long long *tr = P.trace ? P.trace + ((long long)(P.p0 - P.trace_p0) * gridDim.x + blockIdx.x) * 6 : nullptr;
     const bool tracer = tr != nullptr && tid == 0;
 
-    // BULK: all tiles of `buf` have landed (false: gave up -- flag it, bb_device_status reports it)
+    // BULK: all tiles of `buf` have landed.  A thread whose wait gives up flags it (bb_device_status reports it) and
+    // remembers it in `gave_up`; it does NOT leave on its own -- the other warps of the CTA may have seen the tiles and
+    // would wait for it at the next CTA barrier for ever.  The CTA leaves together at that barrier (send_tiles).
+    bool gave_up = false;
     auto tiles_in = [&](int which, unsigned &parity) {
         if (!mbar_wait(sm_mbar + which, parity)) {
             atomicExch(P.status, 2);
-            return false;
+            gave_up = true;
         }
         parity ^= 1u;
         if (tid == 0) mbar_expect_tx(sm_mbar + which, kBufBytes);     // armed again long before the next tiles can come
-        return true;
     };
-    // BULK: the result is back in `own` (in place); tile t goes to CTA t's `theirs`, slot `rank`
+    // BULK: the result is back in `own` (in place); tile t goes to CTA t's `theirs`, slot `rank`.
+    // false: some thread of this CTA gave up waiting for tiles (the same answer in every thread) -- nothing is sent.
     auto send_tiles = [&](cf *own, cf *theirs, int which) {
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // my writes, before the copy engine reads them
-        __syncthreads();
+        if (__syncthreads_or(gave_up)) return false;
         // one copy per tile, spread over the warps (a warp issues its copies one after the other: ~30 ns each from
         // different lanes, ~70 ns each from a loop in one lane)
         constexpr int NW = NT / 32, TPW = (CS + NW - 1) / NW;
@@ -277,6 +280,7 @@ __global__ void __launch_bounds__(SmemC<NX, NY, CS, PT>::NT, 1) bpmc_kernel(cons
         if ((tid & 31) < TPW && t < CS)
             bulk_to_cta(dsmem_addr(theirs + rank * TILE, (unsigned)t), own + t * TILE, kTileBytes,
                         dsmem_addr(sm_mbar + which, (unsigned)t));
+        return true;
     };
 
     Phase16 d = decode_phase16(P, P.p0);
@@ -341,7 +345,7 @@ __global__ void __launch_bounds__(SmemC<NX, NY, CS, PT>::NT, 1) bpmc_kernel(cons
                     const int k = lx.elem(i);
                     rowbuf[(k / W) * TILE + yl * TS + (k % W)] = v[i];
                 }
-                send_tiles(rowbuf, colbuf, 1);
+                if (!send_tiles(rowbuf, colbuf, 1)) break;       // CTA-uniform (the CTA still meets the others below)
             } else {
 #pragma unroll
                 for (int i = 0; i < PT; ++i) {
@@ -381,7 +385,7 @@ __global__ void __launch_bounds__(SmemC<NX, NY, CS, PT>::NT, 1) bpmc_kernel(cons
                     const int k = ly.elem(i);
                     colbuf[(k / R) * TILE + (k % R) * TS + kxl] = v[i];
                 }
-                send_tiles(colbuf, rowbuf, 0);
+                if (!send_tiles(colbuf, rowbuf, 0)) break;
             } else {
 #pragma unroll
                 for (int i = 0; i < PT; ++i) {
@@ -402,7 +406,7 @@ __global__ void __launch_bounds__(SmemC<NX, NY, CS, PT>::NT, 1) bpmc_kernel(cons
             }
             if (tracer) tr[3] = clock64();
             if constexpr (BULK) {
-                if (!(dnx.is_row ? tiles_in(0, par_row) : tiles_in(1, par_col))) break;    // (the CTA still meets the others below)
+                if (dnx.is_row) tiles_in(0, par_row); else tiles_in(1, par_col);
             } else {
                 cluster_wait();
             }

@@ -201,3 +201,60 @@ def test_repeated_runs_are_bit_identical(kc_env):
     assert "bpmc_kernel" in bb.last_kernel()
     for d, I in outs[1:]:
         assert torch.equal(d, outs[0][0]) and torch.equal(I, outs[0][1])
+
+
+def test_summed_intensity_of_a_large_batch_with_a_wide_dynamic_range(oracle_mod, kc_env):
+    """64 clusters add their |u|^2 into the same slices with global float atomics, in whatever order they
+    arrive (bb.h: tolerance contract 1e-4, not bit-reproducible).  Field amplitudes span four decades, so
+    the addends of one pixel span eight: the order of the additions matters as much as it ever will."""
+    bb = kc_env()
+    Nz, B = 12, 64
+    w, dn, f0, nref = problem(oracle_mod, 128, 128, Nz, B, seed=64)
+    amp = np.logspace(-2, 2, B).astype(np.float32)
+    np.random.default_rng(1).shuffle(amp)
+    f0 = (f0 * amp[:, None, None]).astype(np.complex64)
+    d = torch.from_numpy(f0.copy()).cuda()
+    I = torch.full(dn.shape, 7.0, device="cuda")                       # the call zeroes the slices itself
+    bb.propagate(d, dn.cuda(), w.dx, w.dz, w.lam, w.n0, intensity=I, nref=nref)
+    torch.cuda.synchronize()
+    bb.device_status()
+    assert "bpmc_kernel" in bb.last_kernel()
+    Io = np.zeros(dn.shape, dtype=np.float64)
+    for b in range(B):
+        uo, Ib = oracle_mod.propagate(f0[b], dn.numpy(), w.dx, w.dz, w.lam, w.n0, nref=nref)
+        Io += Ib
+        if b in (0, 31, 63):
+            assert rel_l2(d[b].cpu().numpy(), uo) < small_tol(Nz)
+    assert rel_l2(I.cpu().numpy(), Io) < 1e-4
+    # pixel by pixel as well: no slice is dominated by a few lost small addends
+    assert np.abs(I.cpu().numpy() - Io).max() <= 1e-4 * Io.max()
+
+
+def test_a_traced_batch_stays_inside_the_trace_buffer(oracle_mod, kc_env):
+    """bb_probe_trace's buffer has one row per SM.  A batch on the cluster kernel launches 16 CTAs per
+    field -- 12 fields are 192 CTAs, more rows than the buffer has -- so it must run untraced and leave the
+    buffer and the guard words behind it alone; a single field (16 CTAs) is traced."""
+    bb = kc_env()
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    Nz, phases = 4, 16
+    guard = 4096
+    raw = torch.zeros(phases * sms * 6 + guard, dtype=torch.int64, device="cuda")
+    raw[phases * sms * 6:] = -12345
+    buf = raw[:phases * sms * 6].view(phases, sms, 6)
+    try:
+        bb.probe_trace(buf)
+        w, dn, f0, nref = problem(oracle_mod, 128, 128, Nz, 12, seed=3)
+        d = torch.from_numpy(f0.copy()).cuda()
+        bb.propagate(d, dn.cuda(), w.dx, w.dz, w.lam, w.n0, nref=nref)
+        torch.cuda.synchronize()
+        assert "bpmc_kernel" in bb.last_kernel()
+        assert int((raw[phases * sms * 6:] != -12345).sum()) == 0 and int((buf != 0).sum()) == 0
+        uo, _ = oracle_mod.propagate(f0[11], dn.numpy(), w.dx, w.dz, w.lam, w.n0, nref=nref)
+        assert rel_l2(d[11].cpu().numpy(), uo) < small_tol(Nz)
+        d1 = torch.from_numpy(f0[:1].copy()).cuda()
+        bb.propagate(d1, dn.cuda(), w.dx, w.dz, w.lam, w.n0, nref=nref)
+        torch.cuda.synchronize()
+        assert int((buf != 0).sum()) > 0                               # the single field was traced
+        assert int((raw[phases * sms * 6:] != -12345).sum()) == 0
+    finally:
+        bb.probe_trace(None)

@@ -44,12 +44,14 @@ def test_2048_point_lines(oracle_mod, Nx, Ny, Nz, B):
     assert rel_l2(I.cpu().numpy(), Io) < 2 * small_tol(Nz)
 
 
-@pytest.mark.parametrize("Nx,Ny,B,per_field", [(2048, 1024, 2, False), (1024, 2048, 3, True)])
-def test_batches_too_large_for_the_batch_kernel_run_field_by_field(oracle_mod, Nx, Ny, B, per_field):
+@pytest.mark.parametrize("Nx,Ny,B,per_field,Nz", [(2048, 1024, 2, False, 2), (1024, 2048, 3, True, 2),
+                                                  # host runs of more than one z-chunk (chunks of 4 slices on these grids)
+                                                  (2048, 1024, 2, False, 6), (2048, 1024, 2, True, 5)])
+def test_batches_too_large_for_the_batch_kernel_run_field_by_field(oracle_mod, Nx, Ny, B, per_field, Nz):
     """ceil(Ny / SMs) * Nx > 8192: the batch variant cannot hold the screen factors of a CTA's rows; summed and
-    per-field intensities, on top of existing contents (BB_ACCUMULATE)."""
+    per-field intensities, on top of existing contents (BB_ACCUMULATE).  The host-buffer entry point walks the
+    fields inside its chunk loop (each dn chunk is uploaded once) and must give the same bits."""
     bb = need_gpu()
-    Nz = 2
     w, dn, f0 = _case(Nx, Ny, Nz, B, seed=17)
     nref = oracle_mod.nref_from_dn(dn.numpy(), w.n0, 1)
     d = torch.from_numpy(f0).cuda()
@@ -256,7 +258,12 @@ def test_bessel_lattice_matches_oracle(oracle_mod, N, NA_in, NA, M):
 
 
 # ---------------------------------------------------------------- NEXT-3 image formation
-@pytest.mark.parametrize("Nx,Ny,T,G", [(64, 32, 5, 2), (256, 256, 16, 4), (512, 512, 32, 10), (128, 256, 9, 3)])
+@pytest.mark.parametrize("Nx,Ny,T,G", [(64, 32, 5, 2), (256, 256, 16, 4), (512, 512, 32, 10), (128, 256, 9, 3),
+                                       # the kernel's other paths: more emitters in a CTA's halo than it stages (cells of
+                                       # 8 px under 16-px tiles: ~28 owners > 16 slots), more than its 64-entry owner set
+                                       # holds (cells of 4 px: ~72 owners), tiles above the 48 KB default shared memory
+                                       # (T = 64: 6 staged tiles, 152 KB), and T = 96 (one slot: every mixed halo gathers)
+                                       (256, 256, 16, 32), (256, 256, 16, 64), (256, 256, 64, 2), (256, 128, 96, 3)])
 def test_image_formation_matches_oracle(oracle_mod, Nx, Ny, T, G):
     bb = need_gpu()
     rng = np.random.default_rng(T + G)
