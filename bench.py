@@ -182,13 +182,24 @@ def time_config(bb, dev, name, peaks, scratch, per_field=False, runs=10):
         # C4's recipe on 2048 x 1024 pixels -- 2048-point lines (class radix 8)
         import dataclasses
         w = dataclasses.replace(wl.config("C4"), name="P31", Nx=2048, Nz=128, n_cells=500)
+    elif name.startswith("C4x"):
+        # north_star item 4 at the headline size ("100s to 1000s ... PSFs ... within single, highly
+        # multiplexed simulations", many such runs per sample): B multiplexed 1024 x 1024 fields through the shared
+        # 1024^3 volume, summed intensity; field b = C4's emitters with their phases re-drawn from seed b
+        import dataclasses
+        w = dataclasses.replace(wl.config("C4"), name=name, batch=int(name[3:]))
     else:
         w = wl.config(name)
     dn, f0, em = make_inputs(w, dev)
     nref = bb.nref_from_dn(dn, w.n0, w.nref_slab).numpy()
     if em is not None:
         em_d = tuple(t.to(dev) for t in em)
-        src = bb.multiplex_psf(em_d[0], em_d[1], em_d[2], w.NA, w.Nx, w.Ny, w.dx, w.lam)[None].contiguous()
+        fields = []
+        for b in range(w.batch):
+            ph = em_d[1] if b == 0 else torch.from_numpy(
+                np.random.default_rng(1000 + b).uniform(0, 2 * np.pi, size=em[1].shape).astype(np.float32)).to(dev)
+            fields.append(bb.multiplex_psf(em_d[0], ph, em_d[2], w.NA, w.Nx, w.Ny, w.dx, w.lam))
+        src = torch.stack(fields).contiguous()
     else:
         src = torch.from_numpy(f0).to(dev)
 
@@ -206,7 +217,10 @@ def time_config(bb, dev, name, peaks, scratch, per_field=False, runs=10):
     units = float(w.Nx) * w.Ny * w.Nz * B
     out = {"workload": "%s%s: %d field(s) of %dx%d, %d z-slices%s" % (w.name, " per-field intensity" if per_field else "", B, w.Nx, w.Ny, w.Nz,
                                                                      ", %.1f GiB intensity out" % (inten.numel() * 4 / 2**30) if per_field else ""),
-           "baseline_config": ("BASELINE.json configs[%d]" % w.index) if name != "P31" else "none: PAPER.md line 31 grid, C4 recipe",
+           "baseline_config": ("BASELINE.json configs[%d]" % w.index) if name != "P31" and not name.startswith("C4x")
+                              else ("none: PAPER.md line 31 grid, C4 recipe" if name == "P31" else
+                                    "none: BASELINE.json configs[3] volume and emitters, %d fields (north_star item 4)" % B),
+           "us_per_field_z_step": med * 1e3 / w.Nz / B,
            "propagate_ms": med, "propagate_ms_min": mn, "runs": len(ts),
            "value": units / (med * 1e-3) / 1e6, "unit": "Mvox/s", "kernel": bb.last_kernel(),
            "roofline": roofline_fracs(w, med * 1e-3, peaks, per_field)}
@@ -396,29 +410,55 @@ def run_ours(args):
     traffic_note = ("ncu capture of this source digest (profiles/dram_traffic.csv)" if traffic is not None
                     else "null: no ncu capture of the library source being timed (profiles/dram_traffic.csv holds other digests)")
     alu_ach = flop * w.Nz / dur / 1e12
-    result["roofline"] = {"bound": "alu", "achieved": alu_ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
-                          "frac": alu_ach / FP32_PEAK_TFLOPS, "traffic": traffic, "traffic_source": traffic_note,
-                          "kernel": kernel_name, "peak_source": "nominal 148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md)",
-                          "algorithmic_flop_per_launch": flop * w.Nz}
     hbm_ach = hbm_b * w.Nz / dur / 1e9
+    t_step = dur / w.Nz
+    t_hbm = hbm_b / (hbm_peak * 1e9)
+    # fraction of the roofline = T_roof / T per z-step, T_roof = max(T_HBM, T_L2).  `roofline` is that bound
+    # (the L2 one whenever the in-run L2 probe ran, as it binds on every grid: 6 x the HBM bytes at ~2 x the bandwidth);
+    # the HBM and FP32 views follow as roofline_hbm / roofline_alu.
+    result["roofline"] = {"bound": "hbm", "achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s",
+                          "frac": t_hbm / t_step, "traffic": traffic, "traffic_source": traffic_note,
+                          "kernel": kernel_name, "peak_source": hbm_src,
+                          "algorithmic_bytes_per_launch": hbm_b * w.Nz, "us_per_z_step": t_step * 1e6,
+                          "definition": "SURVEY 8d: T_roof / T per z-step, T_roof = max(T_HBM, T_L2); L2 probe not run: HBM bound only"}
     result["roofline_hbm"] = {"bound": "hbm", "achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s",
                               "frac": hbm_ach / hbm_peak, "traffic": traffic, "peak_source": hbm_src,
                               "algorithmic_bytes_per_launch": hbm_b * w.Nz}
+    result["roofline_alu"] = {"bound": "alu", "achieved": alu_ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+                              "frac": alu_ach / FP32_PEAK_TFLOPS,
+                              "peak_source": "nominal FMA peak: 148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md); the transforms are "
+                                             "two-thirds additions, so the ceiling for this instruction mix is about half of it",
+                              "algorithmic_flop_per_launch": flop * w.Nz}
     if rank == 0 and not args.no_probe:
         try:
             peaks["l2_copy"] = bb.probe_l2_bandwidth(32 << 20, 200, 0)
             peaks["l2_read"] = bb.probe_l2_bandwidth(32 << 20, 200, 1)
             fp32_meas = bb.probe_fp32(20000, False)
             l2_ach = l2_b * w.Nz / dur / 1e9
+            t_l2 = l2_b / (peaks["l2_copy"] * 1e9)
             result["roofline_l2"] = {"bound": "l2", "achieved": l2_ach, "peak": peaks["l2_copy"], "unit": "GB/s",
                                      "frac": l2_ach / peaks["l2_copy"],
                                      "peak_read_only": peaks["l2_read"], "frac_vs_read_peak": l2_ach / peaks["l2_read"],
                                      "peak_source": "measured now: bb_probe_l2_bandwidth, 32 MiB resident, copy (half read, half "
                                                     "write, like the field's traffic) and read-only",
                                      "algorithmic_bytes_per_launch": l2_b * w.Nz}
-            result["roofline"]["peak_measured_fma_loop"] = fp32_meas
-            t_roof = max(hbm_b / (hbm_peak * 1e9), l2_b / (peaks["l2_copy"] * 1e9))
-            result["hbm_l2_roofline_frac"] = t_roof / (dur / w.Nz)       # T_roof / T_measured per slice
+            result["roofline_alu"]["peak_measured_fma_loop"] = fp32_meas
+            mix = bb.probe_fp32(4000, 2)
+            result["roofline_alu"]["peak_butterfly_mix"] = mix
+            result["roofline_alu"]["frac_vs_mix_peak"] = alu_ach / mix
+            result["roofline_alu"]["mix_note"] = ("bb_probe_fp32 mode 2: the kernel's own butterflies of a 1024-point phase from registers, "
+                                                  "no memory, at the kernel's occupancy, in SURVEY 8d's flop count; T_ALU at that rate = "
+                                                  "%.2f us per z-step" % (flop / (mix * 1e12) * 1e6))
+            t_roof = max(t_hbm, t_l2)
+            if t_l2 >= t_hbm:
+                result["roofline"].update({"bound": "l2", "achieved": l2_ach, "peak": peaks["l2_copy"],
+                                           "peak_source": result["roofline_l2"]["peak_source"],
+                                           "algorithmic_bytes_per_launch": l2_b * w.Nz})
+            result["roofline"].update({"frac": t_roof / t_step, "t_roof_us_per_z_step": t_roof * 1e6,
+                                       "t_hbm_us_per_z_step": t_hbm * 1e6, "t_l2_us_per_z_step": t_l2 * 1e6,
+                                       "definition": "SURVEY 8d: T_roof / T per z-step, T_roof = max(T_HBM, T_L2); `traffic` is the "
+                                                     "kernel's DRAM bytes per launch (ncu), to be held against roofline_hbm"})
+            result["hbm_l2_roofline_frac"] = t_roof / t_step             # the same number (key kept from rounds 1-2)
         except Exception as e:                                            # noqa: BLE001
             result["roofline_l2"] = {"error": str(e)}
 
@@ -477,7 +517,8 @@ def run_ours(args):
         torch.cuda.empty_cache()
         scratch = torch.zeros(64 << 20, dtype=torch.float32, device=dev)          # 256 MiB
         cfgs = []
-        for name, per_field in (("C1", False), ("C2", False), ("C3", False), ("C5", False), ("C5", True), ("P31", False)):
+        for name, per_field in (("C1", False), ("C2", False), ("C3", False), ("C5", False), ("C5", True), ("P31", False),
+                                ("C4x4", False), ("C4x8", False)):
             try:
                 cfgs.append(time_config(bb, dev, name, peaks, scratch, per_field=per_field))
             except Exception as e:                                        # noqa: BLE001

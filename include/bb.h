@@ -258,7 +258,11 @@ int bb_device_status(void);             /* synchronises the device; BB_ERR_INTER
  * not hold.  Synchronous; allocate and free their own buffers; not used by the BPM path.
  * bb_probe_l2_bandwidth: GB/s over a `bytes`-sized buffer that stays in L2 (mode 0: copy, counts
  * bytes read + written; mode 1: read only).  bb_probe_fp32: TFLOP/s of dependent-free FMA chains,
- * packed = 0 scalar FFMA, 1 = FFMA2 (fma.rn.f32x2).
+ * packed = 0 scalar FFMA, 1 = FFMA2 (fma.rn.f32x2); packed = 2: the library's own butterflies of one
+ * phase of a 1024-point line (radix-16, twiddles, radix-16, radix-4 class step, pointwise multiply, and
+ * back) run from registers with no memory access at the occupancy of the 16-point-thread kernel, credited
+ * with SURVEY 8d's 120 flop per point and phase -- the FP32 ceiling of this instruction mix, against which
+ * the kernel's algorithmic flop rate can be held.
  */
 int bb_probe_l2_bandwidth(unsigned long long bytes, int iters, int mode, double *gb_per_s);
 int bb_probe_fp32(int iters, int packed, double *tflops);

@@ -300,10 +300,11 @@ def probe_l2_bandwidth(nbytes: int = 32 << 20, iters: int = 200, mode: int = 0) 
     return out.value
 
 
-def probe_fp32(iters: int = 20000, packed: bool = False) -> float:
-    """TFLOP/s of the scalar or packed FP32 FMA pipe; see ``bb_probe_fp32``."""
+def probe_fp32(iters: int = 20000, packed=False) -> float:
+    """TFLOP/s of the scalar (``packed`` False / 0) or packed (True / 1) FP32 FMA pipe, or of the library's butterfly
+    mix run from registers (2); see ``bb_probe_fp32``."""
     out = ctypes.c_double()
-    _check(load().bb_probe_fp32(iters, 1 if packed else 0, ctypes.byref(out)))
+    _check(load().bb_probe_fp32(iters, int(packed), ctypes.byref(out)))
     return out.value
 
 

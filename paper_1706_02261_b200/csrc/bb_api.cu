@@ -15,6 +15,8 @@
 #include <string>
 #include <vector>
 
+extern char **environ;
+
 namespace {
 
 using bb::KParams;
@@ -156,12 +158,33 @@ size_t table_budget_bytes() {
     return mb << 20;
 }
 
+// The diagnostic switches the library reads from the environment when it makes a plan.  A BB_* variable that is
+// not one of them is a spelling mistake that would otherwise be ignored without a word: the call fails instead.
+const char *const kEnvSwitches[] = {"BB_TABLE_CACHE_MB", "BB_DISABLE_K16", "BB_DISABLE_K8", "BB_USE_K8", "BB_DISABLE_KC",
+                                    "BB_KC_MODE", "BB_KC_PT", "BB_KC_FORCE", "BB_KC_CS", "BB_K16_NOTMA", "BB_K16_NOPRUNE",
+                                    "BB_K16_CW", "BB_GRID"};
+int check_env_switches() {
+    for (char **e = environ; e && *e; ++e) {
+        if (strncmp(*e, "BB_", 3) != 0) continue;
+        const char *eq = strchr(*e, '=');
+        const size_t n = eq ? (size_t)(eq - *e) : strlen(*e);
+        bool known = false;
+        for (const char *k : kEnvSwitches) known = known || (strlen(k) == n && strncmp(k, *e, n) == 0);
+        if (!known) return fail(BB_ERR_INVALID_ARG, "unknown environment switch %.*s (the library knows BB_TABLE_CACHE_MB, "
+                                "BB_DISABLE_K16/K8/KC, BB_USE_K8, BB_KC_MODE/PT/FORCE/CS, BB_K16_NOTMA/NOPRUNE/CW, BB_GRID)",
+                                (int)n, *e);
+    }
+    return BB_OK;
+}
+
 int get_plan(int Nx, int Ny, Plan **out) {
     int dev, sms;
     int rc = check_arch(&dev, &sms);
     if (rc) return rc;
     for (Plan *p : g_plans)
         if (p->device == dev && p->Nx == Nx && p->Ny == Ny) { *out = p; return BB_OK; }
+    rc = check_env_switches();
+    if (rc) return rc;
     Plan *p = new Plan();
     struct Guard { Plan *p; ~Guard() { if (p) destroy_plan(p); } } guard{p};   // every early return releases what was allocated
     p->device = dev; p->Nx = Nx; p->Ny = Ny; p->sm_count = sms;
@@ -422,6 +445,7 @@ bool make_field_tmap(CUtensorMap *tm, void *field, int Nx, int Ny, int B, int cw
     cuuint32_t box[4] = {(cuuint32_t)cw, 1, 256, 1};
     cuuint32_t estr[4] = {1, 1, 1, 1};
     return fn(tm, CU_TENSOR_MAP_DATA_TYPE_UINT64, 4, field, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+              // L2 promotion: NONE; 64 / 128 / 256 B measured on C4 (round 3): 13.626 / 13.630 / 13.642 ms against 13.627 -- no effect
               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 

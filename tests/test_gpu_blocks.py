@@ -124,3 +124,19 @@ def test_nref_from_dn(oracle_mod, slab):
     const = torch.full((6, 64, 32), 0.02, device="cuda")
     assert np.array_equal(bb.nref_from_dn(const, 1.33, 4).numpy(),
                           np.full(6, np.float32(np.float64(np.float32(1.33)) + np.float64(np.float32(0.02)))))
+
+
+def test_a_misspelt_environment_switch_is_rejected(monkeypatch):
+    """The diagnostic BB_* switches are read when a plan is made; a BB_* name the library does not know fails
+    the call (it would otherwise be ignored silently), and the message names it."""
+    bb = need_gpu()
+    bb.shutdown()
+    monkeypatch.setenv("BB_DISABLE_K61", "1")
+    f = torch.zeros((1, 256, 256), dtype=torch.complex64, device="cuda")
+    with pytest.raises(bb.BBError) as e:
+        bb.fft2(f, -1)
+    assert e.value.status == 1 and "BB_DISABLE_K61" in str(e.value)
+    monkeypatch.delenv("BB_DISABLE_K61")
+    bb.fft2(f, -1)
+    torch.cuda.synchronize()
+    bb.shutdown()
