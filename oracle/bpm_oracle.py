@@ -25,17 +25,28 @@ _f32p = ctypes.POINTER(ctypes.c_float)
 _f64p = ctypes.POINTER(ctypes.c_double)
 
 
-def build(force: bool = False) -> str:
-    """Compile ``bpm_oracle.c`` into ``oracle/liboracle.so`` with gcc (IEEE double, OpenMP)."""
-    if (not force and os.path.exists(_LIB)
-            and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
-        return _LIB
-    tmp = _LIB + ".tmp%d" % os.getpid()
-    cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp",
+def build(force: bool = False, sanitize: bool | None = None) -> str:
+    """Compile ``bpm_oracle.c`` into ``oracle/liboracle.so`` with gcc (IEEE double, OpenMP).
+
+    ``sanitize`` (default: the environment variable ``ORACLE_SANITIZE=1``) builds ``liboracle_san.so`` with
+    AddressSanitizer and UndefinedBehaviorSanitizer instead -- same source, same
+    floating-point flags; run the CPU tests against it as
+    ``ORACLE_SANITIZE=1 LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 pytest -m "not gpu"``.
+    """
+    if sanitize is None:
+        sanitize = os.environ.get("ORACLE_SANITIZE", "") == "1"
+    lib = os.path.join(_HERE, "liboracle_san.so") if sanitize else _LIB
+    if (not force and os.path.exists(lib)
+            and os.path.getmtime(lib) >= os.path.getmtime(_SRC)):
+        return lib
+    tmp = lib + ".tmp%d" % os.getpid()
+    opt = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"] \
+        if sanitize else ["-O2"]
+    cmd = ["gcc", *opt, "-std=c11", "-fPIC", "-shared", "-fopenmp",
            "-ffp-contract=off", "-fno-fast-math", "-o", tmp, _SRC, "-lm"]
     subprocess.run(cmd, check=True)
-    os.replace(tmp, _LIB)
-    return _LIB
+    os.replace(tmp, lib)
+    return lib
 
 
 def _load():
